@@ -1,0 +1,125 @@
+/* lrmd.h — C ABI of the B200 (sm_100a) long-range molecular-dynamics hot path.
+ *
+ * What it computes: the data-parallel hot path of arXiv 1212.0262 (T. M. Rocha Filho,
+ * "Molecular dynamics for long-range interacting systems on Graphic Processing Units"):
+ * force evaluation, fused kick/drift updates and energy sums of the fourth-order symplectic
+ * integrator for three N-body models of unit-mass particles (PAPER.md = /root/reference/PAPER.md):
+ *
+ *   LRMD_HMF     H = 1/2 sum p_i^2 + (1/N) sum_{i<j} [1 - cos(th_i - th_j)]            PAPER.md:36 eq.(2)
+ *   LRMD_RING    H = 1/2 sum p_i^2 - (1/N) sum_{i<j} 1/(sqrt2 sqrt(1 - cos(th_i-th_j) + eps))   PAPER.md:29 eq.(1)
+ *   LRMD_GRAV2D  H = 1/2 sum (px_i^2 + py_i^2) + (1/N) sum_{i<j} log[(x_i-x_j)^2 + (y_i-y_j)^2 + eps]   PAPER.md:40 eq.(3)
+ *
+ * Forces are f = -dH/dq:
+ *   HMF     f_i = cos(th_i) My - sin(th_i) Mx, (Mx,My) = (1/N) sum (cos th_j, sin th_j)   PAPER.md:73-77 eqs.(6)-(7)
+ *   RING    f_i = -(1/(2 sqrt2 N)) sum_j (s_i c_j - c_i s_j) / (1 + eps - c_i c_j - s_i s_j)^(3/2)
+ *           PAPER.md:88,97 eqs.(8)-(9); the sign is that of -dH/dtheta (eq.(8) prints the opposite
+ *           sign; reading G1)
+ *   GRAV2D  F_i = -(2/N) sum_j (r_i - r_j) / (|r_i - r_j|^2 + eps)                       PAPER.md:110, from eq.(3)
+ *
+ * One time step is Yoshida's composition, eq.(4) and the 12-step listing
+ * PAPER.md:54-62 (readings G2-G4): with f = F(q) cached,
+ *   p += B0 dt f; q += D0 dt p; f = F(q);  p += B1 dt f; q += D1 dt p; f = F(q);
+ *   p += B1 dt f; q += D0 dt p; f = F(q);  p += B0 dt f            (f is kept for the next step)
+ * i.e. three force evaluations per step, 3n+1 for n steps from a fresh state.
+ *
+ * Conventions
+ *   - All array arguments are DEVICE pointers to contiguous fp64 arrays of length N on the
+ *     current CUDA device, 16-byte aligned, owned by the caller.  The only HOST pointers are
+ *     `out`, `bytes` and the const char* returned by lrmd_strerror.
+ *   - The library never allocates device memory: scratch comes from lrmd_set_workspace().
+ *   - Work is enqueued on the given CUDA stream (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream) and the call returns without synchronising, except where stated.
+ *   - Every call returns LRMD_OK (0) or a negative error code; nothing throws, prints or exits.
+ *   - Calls on one context are not thread-safe; different contexts are independent.
+ *   - Results are bitwise reproducible run to run for fixed (model, N, eps, options): all
+ *     reductions use fixed trees and there are no floating-point atomics.
+ */
+#ifndef LRMD_H_
+#define LRMD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lrmd_ctx lrmd_ctx;
+
+enum { LRMD_HMF = 0, LRMD_RING = 1, LRMD_GRAV2D = 2 };
+
+enum {
+    LRMD_OK = 0,
+    LRMD_EINVAL = -1,        /* bad argument (NULL, wrong NULL pattern, N < 1, eps <= 0 ...)  */
+    LRMD_ESTATE = -2,        /* state or workspace not set                                     */
+    LRMD_ECUDA = -3,         /* a CUDA call failed; see lrmd_last_cuda_error                   */
+    LRMD_EUNSUPPORTED = -4   /* valid request this build does not implement                    */
+};
+
+/* lrmd_set_option keys */
+enum {
+    LRMD_OPT_PAIR_PRECISION = 0, /* 0 = fp64 pair arithmetic (default); 1 = fp32 pair arithmetic with
+                                    chunked fp32 -> fp64 accumulation (GRAV2D only)      */
+    LRMD_OPT_JSPLIT = 1,         /* pair models: number of j-chunks per i-tile (0 = choose from N)     */
+    LRMD_OPT_GRAPH = 2,          /* 1 = lrmd_step replays a captured CUDA graph of one step (default
+                                    for small N), 0 = plain launches, -1 = choose from N              */
+    LRMD_OPT_HMF_GRID = 3        /* HMF: number of CTAs of the fused substage kernel (0 = choose)      */
+};
+
+/* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.
+ * eps: softening of eqs.(1),(3); ignored for HMF; must be finite and > 0 for RING and GRAV2D
+ * (the pair kernels include the j = i term, which is exactly zero only for eps > 0 — the
+ * paper's tile loop does the same).  The library owns *out (host memory only). */
+int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps);
+
+/* Free the context (host memory only; device buffers belong to the caller). NULL is LRMD_EINVAL. */
+int lrmd_destroy(lrmd_ctx* ctx);
+
+/* Scratch needed for the current options: partial sums, the packed j-stream (cos,sin) or (x,y)
+ * of PAPER.md:100, partial forces, device scalars.  Query, allocate `*bytes` on the device
+ * (256-byte aligned), then bind it.  Changing an option that alters the size returns the
+ * context to "workspace not set".  The contents are private to the library. */
+int lrmd_workspace_bytes(const lrmd_ctx* ctx, size_t* bytes);
+int lrmd_set_workspace(lrmd_ctx* ctx, void* device_ptr, size_t bytes, void* cuda_stream);
+
+/* Bind the state arrays, updated IN PLACE by lrmd_step.
+ *   HMF, RING: (theta, p, NULL, NULL);   GRAV2D: (x, y, px, py).
+ * Any other NULL pattern is LRMD_EINVAL.  Binding invalidates the cached force: call it again
+ * after modifying the arrays yourself.  Angles are never wrapped (reading G8). */
+int lrmd_set_state(lrmd_ctx* ctx, double* a0, double* a1, double* a2, double* a3);
+
+/* Advance n >= 0 full steps of size dt (may be negative) of eq.(4).  n = 0 is a no-op. */
+int lrmd_step(lrmd_ctx* ctx, int64_t n, double dt, void* cuda_stream);
+
+/* Write the force at the current positions: f0 = f (HMF, RING; f1 must be NULL) or
+ * (f0, f1) = (fx, fy) (GRAV2D).  Uses the cached force if valid, else evaluates and caches it. */
+int lrmd_forces(lrmd_ctx* ctx, double* f0, double* f1, void* cuda_stream);
+
+/* Write out4[0..3] = {K, V, a, b} (DEVICE pointer to 4 doubles):
+ *   K = 1/2 sum p^2;  V = the potential energy of eqs.(1)-(3)
+ *   (HMF: V = (N/2)(1 - Mx^2 - My^2), eq.(5); RING, GRAV2D: O(N^2) pair sum over i<j);
+ *   (a, b) = (Mx, My) for HMF, (sum p, 0) for RING, (sum px, sum py) for GRAV2D. */
+int lrmd_energy(lrmd_ctx* ctx, double* out4_device, void* cuda_stream);
+
+/* Set an option (keys above).  Unknown key or bad value: LRMD_EINVAL. */
+int lrmd_set_option(lrmd_ctx* ctx, int key, int64_t value);
+/* Read back an option as resolved for this context (e.g. the j-split chosen from N). */
+int lrmd_get_option(const lrmd_ctx* ctx, int key, int64_t* value);
+
+/* Number of kernel launches (graph kernel nodes counted individually) enqueued by this context
+ * since creation: the caller's evidence that the CUDA path ran. */
+int lrmd_launch_count(const lrmd_ctx* ctx, int64_t* launches);
+
+/* The cudaError_t (as int) of the last failed CUDA call on this context, 0 if none. */
+int lrmd_last_cuda_error(const lrmd_ctx* ctx);
+
+/* Static string for an error code. Never NULL. */
+const char* lrmd_strerror(int code);
+
+/* Yoshida coefficients used by lrmd_step: out4_host = {B0, B1, D0, D1} (HOST pointer). */
+int lrmd_coefficients(double* out4_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LRMD_H_ */

@@ -1,0 +1,109 @@
+// common.cuh — device helpers shared by the lrmd kernels (sm_100a only).
+//   * deterministic warp/block reductions (fixed shuffle trees, no atomics)
+//   * mbarrier + 1-D TMA bulk copy (cp.async.bulk -> SASS UBLKCP) wrappers
+//   * approximate fp64 reciprocal / reciprocal square root seeds (MUFU.RCP64H / MUFU.RSQ64H)
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "lrmd kernels are written for sm_100a (B200) only"
+#endif
+
+namespace lrmd {
+
+constexpr int kWarp = 32;
+
+// ---- reductions -------------------------------------------------------------------------------
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum NV values per thread over a block of THREADS threads.  Result valid in ALL threads
+// (broadcast through shared memory).  Order is fixed: xor-shuffle tree inside each warp, then
+// warp sums added in warp-index order.  `scratch` must hold NV * (THREADS/32) doubles and
+// may be reused after the call returns (the function ends with a barrier).
+template <int THREADS, int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double* scratch) {
+    constexpr int NW = THREADS / kWarp;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = warp_sum(v[k]);
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) scratch[k * NW + w] = v[k];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double s = scratch[k * NW];
+#pragma unroll
+        for (int i = 1; i < NW; ++i) s += scratch[k * NW + i];
+        v[k] = s;
+    }
+    __syncthreads();
+}
+
+// ---- mbarrier / TMA 1-D bulk copy ----------------------------------------------------------------
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// global -> shared::cta bulk copy of `bytes` (multiple of 16; both addresses 16-byte aligned),
+// completion signalled on `bar` (complete_tx).
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- fp64 seeds ------------------------------------------------------------------------------------
+
+// ~20-bit 1/x from the high word of x (MUFU.RCP64H); x must be a positive normal number.
+__device__ __forceinline__ double rcp_seed(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+// ~20-bit 1/sqrt(x) (MUFU.RSQ64H); x must be a positive normal number.
+__device__ __forceinline__ double rsqrt_seed(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+}  // namespace lrmd

@@ -1,0 +1,210 @@
+// hmf_kernels.cuh — HMF model (section 3.1), HBM-bandwidth-bound path.
+//
+// One fused kernel per integrator substage (SURVEY.md 8(a) rows a-H1..a-H3):
+//     (Mx,My) <- (1/N) * sum of the previous kernel's per-CTA partial sums        eq.(7)
+//     s,c = sincos(theta_i);  f_i = c*My - s*Mx                                    eq.(6)
+//     p_i += kickA*f_i [; p_i += kickB*f_i]                                        listing steps 2,5,8,11
+//     theta_i += drift*p_i                                                         listing steps 3,6,9
+//     s',c' = sincos(theta_i);  per-CTA partial (sum c', sum s') -> partial_out    eq.(7) at the new angles
+// so every substage streams theta and p through HBM exactly once (32 B per particle: 16 read,
+// 16 written in place).  The paper stores cos/sin in global memory to avoid recomputing them
+// (PAPER.md:80); on B200 recomputing (20 FP64 instructions) is cheaper than +32 B per particle.
+//
+// Determinism: the grid size G is fixed per context; every thread visits a fixed set of
+// particles in a fixed order, block sums use fixed trees, and the G partials are summed in a
+// fixed order by EVERY CTA of the consuming kernel (no atomics, no "last block" ticket, no
+// fences) — all CTAs therefore get bit-identical (Mx, My).
+#pragma once
+
+#include "common.cuh"
+#include "trig.cuh"
+
+namespace lrmd {
+
+constexpr int kHmfThreads = 256;
+constexpr int kHmfMaxGrid = 148 * 8;
+
+struct alignas(32) dbl4 { double a, b, c, d; };
+
+__device__ __forceinline__ dbl4 ld256(const double* p) {
+    dbl4 v;
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.a), "=d"(v.b), "=d"(v.c), "=d"(v.d) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st256(double* p, const dbl4& v) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.a), "d"(v.b), "d"(v.c), "d"(v.d) : "memory");
+}
+
+// (Mx, My) from the producer's partial sums; identical in every thread of every CTA.
+template <int THREADS>
+__device__ __forceinline__ void hmf_magnetisation(const double2* __restrict__ partial_in, int g_in, double inv_n,
+                                                  double* scratch, double& Mx, double& My) {
+    double v[2] = {0.0, 0.0};
+    for (int i = threadIdx.x; i < g_in; i += THREADS) {
+        const double2 q = partial_in[i];
+        v[0] += q.x;
+        v[1] += q.y;
+    }
+    block_sum<THREADS, 2>(v, scratch);
+    Mx = v[0] * inv_n;
+    My = v[1] * inv_n;
+}
+
+template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
+__device__ __forceinline__ void hmf_particle(double& th, double& p, double Mx, double My, double kickA, double kickB,
+                                             double drift, double& accC, double& accS) {
+    if (KICK) {
+        double s, c;
+        sincos_pi4(th, s, c);
+        const double f = fma(c, My, -(s * Mx));
+        p = fma(kickA, f, p);
+        if (KICK2) p = fma(kickB, f, p);
+    }
+    if (DRIFT) th = fma(drift, p, th);
+    if (REDUCE) {
+        double s, c;
+        sincos_pi4(th, s, c);
+        accC += c;
+        accS += s;
+    }
+}
+
+// KICK: apply p += kickA f (and kickB f if KICK2) with M from partial_in.
+// DRIFT: theta += drift p.   REDUCE: write per-CTA (sum cos, sum sin) of the final angles.
+template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
+__global__ void __launch_bounds__(kHmfThreads)
+hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double kickA, double kickB,
+                    double drift, const double2* __restrict__ partial_in, int g_in, double2* __restrict__ partial_out) {
+    __shared__ double scratch[2 * (kHmfThreads / 32)];
+    const long long nvec = N >> 2;
+    const long long stride = (long long)gridDim.x * kHmfThreads;
+    long long v = (long long)blockIdx.x * kHmfThreads + threadIdx.x;
+
+    // issue the first loads before the (latency-bound) magnetisation prologue
+    dbl4 t4 = {0, 0, 0, 0}, p4 = {0, 0, 0, 0};
+    const bool have = v < nvec;
+    if (have) {
+        t4 = ld256(theta + 4 * v);
+        if (KICK || DRIFT) p4 = ld256(p + 4 * v);
+    }
+    double Mx = 0.0, My = 0.0;
+    if (KICK) hmf_magnetisation<kHmfThreads>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+
+    double accC = 0.0, accS = 0.0;
+    while (v < nvec) {
+        const long long vn = v + stride;
+        dbl4 tn = {0, 0, 0, 0}, pn = {0, 0, 0, 0};
+        if (vn < nvec) {   // software prefetch of the next chunk
+            tn = ld256(theta + 4 * vn);
+            if (KICK || DRIFT) pn = ld256(p + 4 * vn);
+        }
+        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.a, p4.a, Mx, My, kickA, kickB, drift, accC, accS);
+        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.b, p4.b, Mx, My, kickA, kickB, drift, accC, accS);
+        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.c, p4.c, Mx, My, kickA, kickB, drift, accC, accS);
+        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.d, p4.d, Mx, My, kickA, kickB, drift, accC, accS);
+        if (DRIFT) st256(theta + 4 * v, t4);
+        if (KICK) st256(p + 4 * v, p4);
+        t4 = tn;
+        p4 = pn;
+        v = vn;
+    }
+    // ragged tail: N % 4 particles, one per thread of the lowest global thread ids
+    {
+        const long long g = (long long)blockIdx.x * kHmfThreads + threadIdx.x;
+        const long long i = (nvec << 2) + g;
+        if (g < 4 && i < N) {
+            double th = theta[i], pp = (KICK || DRIFT) ? p[i] : 0.0;
+            hmf_particle<KICK, KICK2, DRIFT, REDUCE>(th, pp, Mx, My, kickA, kickB, drift, accC, accS);
+            if (DRIFT) theta[i] = th;
+            if (KICK) p[i] = pp;
+        }
+    }
+    if (REDUCE) {
+        double r[2] = {accC, accS};
+        block_sum<kHmfThreads, 2>(r, scratch);
+        if (threadIdx.x == 0) partial_out[blockIdx.x] = make_double2(r[0], r[1]);
+    }
+}
+
+// f_i = cos(theta_i) My - sin(theta_i) Mx  -> f   (lrmd_forces; eq.(6))
+__global__ void __launch_bounds__(kHmfThreads)
+hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long long N,
+                 const double2* __restrict__ partial_in, int g_in) {
+    __shared__ double scratch[2 * (kHmfThreads / 32)];
+    double Mx, My;
+    hmf_magnetisation<kHmfThreads>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+    const long long stride = (long long)gridDim.x * kHmfThreads;
+    for (long long i = (long long)blockIdx.x * kHmfThreads + threadIdx.x; i < N; i += stride) {
+        double s, c;
+        sincos_pi4(theta[i], s, c);
+        f[i] = fma(c, My, -(s * Mx));
+    }
+}
+
+// Per-CTA partial sums of up to two arrays: (sum a^2 [+ b^2], sum a, sum b) -> part[3*blockIdx..]
+// Used for K = 1/2 sum p^2 and the total momentum of all three models.
+__global__ void __launch_bounds__(kHmfThreads)
+kinetic_partial_kernel(const double* __restrict__ a, const double* __restrict__ b, long long N,
+                       double* __restrict__ part) {
+    __shared__ double scratch[3 * (kHmfThreads / 32)];
+    double r[3] = {0.0, 0.0, 0.0};
+    const long long stride = (long long)gridDim.x * kHmfThreads;
+    for (long long i = (long long)blockIdx.x * kHmfThreads + threadIdx.x; i < N; i += stride) {
+        const double x = a[i];
+        r[0] = fma(x, x, r[0]);
+        r[1] += x;
+        if (b) {
+            const double y = b[i];
+            r[0] = fma(y, y, r[0]);
+            r[2] += y;
+        }
+    }
+    block_sum<kHmfThreads, 3>(r, scratch);
+    if (threadIdx.x == 0) {
+        part[3 * blockIdx.x + 0] = r[0];
+        part[3 * blockIdx.x + 1] = r[1];
+        part[3 * blockIdx.x + 2] = r[2];
+    }
+}
+
+// One CTA: out4 = {K, V, a, b}.
+//   kpart: g_k triples from kinetic_partial_kernel.
+//   HMF (model 0): mpart = g_m (sum cos, sum sin) partials; V = (N/2)(1 - Mx^2 - My^2), eq.(5) PAPER.md:69;
+//                  (a, b) = (Mx, My).
+//   pair models:   vpart = g_v partial sums of the pair-potential kernel, already scaled; V = sum;
+//                  (a, b) = total momentum.
+__global__ void __launch_bounds__(kHmfThreads)
+energy_finalize_kernel(int model, long long N, const double* __restrict__ kpart, int g_k,
+                       const double2* __restrict__ mpart, int g_m, const double* __restrict__ vpart, int g_v,
+                       double* __restrict__ out4) {
+    __shared__ double scratch[3 * (kHmfThreads / 32)];
+    double r[3] = {0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < g_k; i += kHmfThreads) {
+        r[0] += kpart[3 * i];
+        r[1] += kpart[3 * i + 1];
+        r[2] += kpart[3 * i + 2];
+    }
+    block_sum<kHmfThreads, 3>(r, scratch);
+    const double K = 0.5 * r[0];
+    double V, a = r[1], b = r[2];
+    if (model == 0) {
+        double Mx, My;
+        hmf_magnetisation<kHmfThreads>(mpart, g_m, 1.0 / (double)N, scratch, Mx, My);
+        V = 0.5 * (double)N * (1.0 - Mx * Mx - My * My);
+        a = Mx;
+        b = My;
+    } else {
+        double v[1] = {0.0};
+        for (int i = threadIdx.x; i < g_v; i += kHmfThreads) v[0] += vpart[i];
+        block_sum<kHmfThreads, 1>(v, scratch);
+        V = v[0];
+    }
+    if (threadIdx.x == 0) {
+        out4[0] = K;
+        out4[1] = V;
+        out4[2] = a;
+        out4[3] = b;
+    }
+}
+
+}  // namespace lrmd

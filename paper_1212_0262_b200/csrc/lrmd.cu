@@ -1,0 +1,543 @@
+// lrmd.cu — the C ABI of include/lrmd.h: argument validation, workspace layout, integrator
+// substage sequencing (eq.(4) and the 12-step listing) and kernel launches.
+// All arithmetic of the method runs in the kernels of hmf_kernels.cuh / pair_kernels.cuh; the
+// host only computes the four products B*dt, D*dt per call and chooses launch shapes.
+#include "../../include/lrmd.h"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <tuple>
+#include <utility>
+
+#include "hmf_kernels.cuh"
+#include "pair_kernels.cuh"
+
+namespace {
+
+using namespace lrmd;
+
+constexpr int kNumSm = 148;                 // B200
+constexpr size_t kAlign = 256;
+constexpr int kEnergyGrid = kNumSm * 4;     // CTAs of the kinetic-energy partial kernel
+constexpr int kGraphSteps = 8;              // steady-state steps per replayed CUDA graph
+
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t hmf_partial = 0;   // 3 rotating buffers of kHmfMaxGrid double2 (HMF)
+    size_t js = 0;            // packed j-stream double2[N] (pair models)
+    size_t partial0 = 0;      // [S][N] partial forces
+    size_t partial1 = 0;      // [S][N] (GRAV2D)
+    size_t kpart = 0;         // 3 * kEnergyGrid
+    size_t vpart = 0;         // S * itiles (pair models)
+    size_t total = 0;
+};
+
+}  // namespace
+
+struct lrmd_ctx {
+    int model = 0;
+    int64_t N = 0;
+    double eps = 0.0;
+    // options as set (0 / -1 = choose)
+    int64_t opt_precision = 0, opt_jsplit = 0, opt_graph = -1, opt_hmf_grid = 0;
+    // resolved
+    int S = 1, itiles = 0, hmf_grid = 0;
+    bool use_graph = false;
+    Layout lay;
+    // bindings
+    char* ws = nullptr;
+    double *a0 = nullptr, *a1 = nullptr, *a2 = nullptr, *a3 = nullptr;
+    bool state_set = false;
+    bool force_valid = false;   // HMF: hmf_partial[cur] holds the sums at theta; pair: partial* hold F(q)
+    bool js_valid = false;      // pair models: js[] matches q
+    int cur = 0;                // HMF: which of the 3 partial buffers is current
+    // cached CUDA graph of kGraphSteps steady-state steps (HMF)
+    cudaGraphExec_t graph_exec = nullptr;
+    double graph_dt = 0.0;
+    int graph_cur = -1;
+    int64_t graph_nodes = 0;
+    // bookkeeping
+    int64_t launches = 0;
+    int cuda_err = 0;
+};
+
+namespace {
+
+// ---- option resolution -------------------------------------------------------------------------------
+
+int choose_jsplit(int64_t N, int itiles) {
+    // Fill the 148 x kPairCtasPerSm resident CTA slots in (nearly) whole waves; keep each j-chunk
+    // at least 1024 elements so the tile pipeline amortises its prologue.
+    const int64_t slots = (int64_t)kNumSm * kPairCtasPerSm;
+    int64_t smax = N / 1024;
+    if (smax < 1) smax = 1;
+    if (smax > 64) smax = 64;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int64_t s = 1; s <= smax; ++s) {
+        const int64_t ctas = (int64_t)itiles * s;
+        const int64_t waves = (ctas + slots - 1) / slots;
+        const double eff = (double)ctas / (double)(waves * slots);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = (int)s; }
+        if (eff >= 0.97) break;
+    }
+    return best;
+}
+
+void resolve(lrmd_ctx* c) {
+    const int64_t N = c->N;
+    Layout L;
+    size_t off = 0;
+    if (c->model == LRMD_HMF) {
+        const int64_t nvec = N >> 2;
+        int64_t g = c->opt_hmf_grid > 0 ? c->opt_hmf_grid : (nvec + kHmfThreads - 1) / kHmfThreads;
+        if (g < 1) g = 1;
+        if (g > kHmfMaxGrid) g = kHmfMaxGrid;
+        c->hmf_grid = (int)g;
+        c->S = 1;
+        c->itiles = 0;
+        L.hmf_partial = off; off = align_up(off + 3 * sizeof(double2) * kHmfMaxGrid);
+        c->use_graph = c->opt_graph < 0 ? (N <= (1 << 20)) : (c->opt_graph != 0);
+    } else {
+        c->itiles = (int)((N + kPairITile - 1) / kPairITile);
+        c->S = c->opt_jsplit > 0 ? (int)c->opt_jsplit : choose_jsplit(N, c->itiles);
+        if ((int64_t)c->S > N) c->S = (int)N;
+        c->hmf_grid = 0;
+        L.js = off; off = align_up(off + sizeof(double2) * (size_t)N);
+        L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->S);
+        if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->S); }
+        L.vpart = off; off = align_up(off + sizeof(double) * (size_t)c->S * c->itiles);
+        c->use_graph = false;
+    }
+    L.kpart = off; off = align_up(off + sizeof(double) * 3 * kEnergyGrid);
+    L.total = off;
+    c->lay = L;
+}
+
+void drop_graph(lrmd_ctx* c) {
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    c->graph_cur = -1;
+    c->graph_nodes = 0;
+}
+
+// ---- launcher: the same call either enqueues on a stream or appends a kernel node to a graph ---------
+
+struct Launcher {
+    lrmd_ctx* c;
+    cudaStream_t stream;
+    cudaGraph_t graph = nullptr;       // non-null: build mode
+    cudaGraphNode_t last = nullptr;
+    int64_t nodes = 0;
+    int rc = LRMD_OK;
+
+    template <typename... KA, typename... A>
+    void go(void (*kernel)(KA...), dim3 grid, dim3 block, A... a) {
+        static_assert(sizeof...(KA) == sizeof...(A), "argument count");
+        if (rc != LRMD_OK) return;
+        std::tuple<KA...> vals{static_cast<KA>(a)...};
+        void* ptrs[sizeof...(KA)];
+        fill(ptrs, vals, std::index_sequence_for<KA...>{});
+        cudaError_t e;
+        if (graph) {
+            cudaKernelNodeParams kp;
+            std::memset(&kp, 0, sizeof(kp));
+            kp.func = (void*)kernel;
+            kp.gridDim = grid;
+            kp.blockDim = block;
+            kp.sharedMemBytes = 0;
+            kp.kernelParams = ptrs;
+            cudaGraphNode_t node;
+            e = cudaGraphAddKernelNode(&node, graph, last ? &last : nullptr, last ? 1 : 0, &kp);
+            last = node;
+            ++nodes;
+        } else {
+            e = cudaLaunchKernel((const void*)kernel, grid, block, ptrs, 0, stream);
+            if (e == cudaSuccess) ++c->launches;
+        }
+        if (e != cudaSuccess) {
+            c->cuda_err = (int)e;
+            rc = LRMD_ECUDA;
+            (void)cudaGetLastError();
+        }
+    }
+
+    template <typename T, size_t... I>
+    static void fill(void** ptrs, T& vals, std::index_sequence<I...>) {
+        ((ptrs[I] = (void*)&std::get<I>(vals)), ...);
+    }
+};
+
+inline double2* hmf_buf(lrmd_ctx* c, int k) {
+    return reinterpret_cast<double2*>(c->ws + c->lay.hmf_partial) + (size_t)k * kHmfMaxGrid;
+}
+inline double2* js_ptr(lrmd_ctx* c) { return reinterpret_cast<double2*>(c->ws + c->lay.js); }
+inline double* part0(lrmd_ctx* c) { return reinterpret_cast<double*>(c->ws + c->lay.partial0); }
+inline double* part1(lrmd_ctx* c) {
+    return c->model == LRMD_GRAV2D ? reinterpret_cast<double*>(c->ws + c->lay.partial1) : nullptr;
+}
+inline double* kpart(lrmd_ctx* c) { return reinterpret_cast<double*>(c->ws + c->lay.kpart); }
+inline double* vpart(lrmd_ctx* c) { return reinterpret_cast<double*>(c->ws + c->lay.vpart); }
+
+struct Coef { double B0, B1, D0, D1; };
+Coef coefficients() {
+    // Yoshida's triple jump (reading G4): w1 = 1/(2 - 2^(1/3)), w0 = -2^(1/3)/(2 - 2^(1/3)).
+    const double cb = std::cbrt(2.0);
+    const double w1 = 1.0 / (2.0 - cb), w0 = -cb / (2.0 - cb);
+    return Coef{0.5 * w1, 0.5 * (w0 + w1), w1, w0};
+}
+
+// ---- HMF sequencing ----------------------------------------------------------------------------------
+
+// One fused substage: [kick kickA (+kickB)] -> drift -> reduce into the next partial buffer.
+void hmf_substage(Launcher& L, bool kick2, double kickA, double kickB, double drift, int& cur) {
+    lrmd_ctx* c = L.c;
+    const int nxt = (cur + 1) % 3;
+    const dim3 g(c->hmf_grid), b(kHmfThreads);
+    if (kick2)
+        L.go(hmf_substage_kernel<true, true, true, true>, g, b, c->a0, c->a1, c->N, kickA, kickB, drift,
+             hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
+    else
+        L.go(hmf_substage_kernel<true, false, true, true>, g, b, c->a0, c->a1, c->N, kickA, 0.0, drift,
+             hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
+    cur = nxt;
+}
+
+void hmf_reduce_only(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    L.go(hmf_substage_kernel<false, false, false, true>, dim3(c->hmf_grid), dim3(kHmfThreads), c->a0, c->a1, c->N,
+         0.0, 0.0, 0.0, hmf_buf(c, c->cur), c->hmf_grid, hmf_buf(c, c->cur));
+}
+
+// One full step.  merged: the closing kick B0 dt of the previous step is folded into this
+// step's first substage (same force, two FMAs in the order they would have run separately).
+void hmf_one_step(Launcher& L, const Coef& k, double dt, bool merged, int& cur) {
+    hmf_substage(L, merged, k.B0 * dt, k.B0 * dt, k.D0 * dt, cur);
+    hmf_substage(L, false, k.B1 * dt, 0.0, k.D1 * dt, cur);
+    hmf_substage(L, false, k.B1 * dt, 0.0, k.D0 * dt, cur);
+}
+
+void hmf_closing_kick(Launcher& L, const Coef& k, double dt, int cur) {
+    lrmd_ctx* c = L.c;
+    L.go(hmf_substage_kernel<true, false, false, false>, dim3(c->hmf_grid), dim3(kHmfThreads), c->a0, c->a1, c->N,
+         k.B0 * dt, 0.0, 0.0, hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, cur));
+}
+
+int hmf_build_graph(lrmd_ctx* c, const Coef& k, double dt) {
+    drop_graph(c);
+    cudaGraph_t g;
+    cudaError_t e = cudaGraphCreate(&g, 0);
+    if (e != cudaSuccess) { c->cuda_err = (int)e; return LRMD_ECUDA; }
+    Launcher L{c, nullptr};
+    L.graph = g;
+    int cur = c->cur;
+    for (int s = 0; s < kGraphSteps; ++s) hmf_one_step(L, k, dt, true, cur);
+    int rc = L.rc;
+    if (rc == LRMD_OK) {
+        e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+        if (e != cudaSuccess) { c->cuda_err = (int)e; rc = LRMD_ECUDA; c->graph_exec = nullptr; }
+    }
+    cudaGraphDestroy(g);
+    if (rc == LRMD_OK) { c->graph_dt = dt; c->graph_cur = c->cur; c->graph_nodes = L.nodes; }
+    return rc;
+}
+
+int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
+    const Coef k = coefficients();
+    Launcher L{c, stream};
+    if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }
+    int cur = c->cur;
+    hmf_one_step(L, k, dt, false, cur);     // cur returns to c->cur after 3 substages
+    int64_t left = n - 1;
+    if (L.rc != LRMD_OK) return L.rc;
+    if (c->use_graph && left >= kGraphSteps) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        cudaStreamIsCapturing(stream, &cs);
+        if (cs == cudaStreamCaptureStatusNone) {
+            if (!c->graph_exec || c->graph_dt != dt || c->graph_cur != c->cur) {
+                const int rc = hmf_build_graph(c, k, dt);
+                if (rc != LRMD_OK) return rc;
+            }
+            while (left >= kGraphSteps) {
+                const cudaError_t e = cudaGraphLaunch(c->graph_exec, stream);
+                if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_ECUDA; }
+                c->launches += c->graph_nodes;
+                left -= kGraphSteps;
+            }
+        }
+    }
+    for (; left > 0; --left) hmf_one_step(L, k, dt, true, cur);
+    hmf_closing_kick(L, k, dt, cur);
+    return L.rc;
+}
+
+// ---- pair-model sequencing ---------------------------------------------------------------------------
+
+void pair_pack(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    const dim3 g((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), b(kUpdThreads);
+    if (c->model == LRMD_RING) L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, js_ptr(c));
+    else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, js_ptr(c));
+}
+
+void pair_force(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    const dim3 g((unsigned)c->itiles, (unsigned)c->S), b(kPairThreads);
+    if (c->model == LRMD_RING)
+        L.go(pair_force_kernel<1>, g, b, js_ptr(c), c->N, c->eps, -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N),
+             part0(c), part1(c));
+    else
+        L.go(pair_force_kernel<2>, g, b, js_ptr(c), c->N, c->eps, -2.0 / (double)c->N, part0(c), part1(c));
+}
+
+void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB, double d) {
+    lrmd_ctx* c = L.c;
+    const dim3 g((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), b(kUpdThreads);
+    double *q0 = c->a0, *q1 = nullptr, *p0 = c->a1, *p1 = nullptr;
+    if (c->model == LRMD_GRAV2D) { q1 = c->a1; p0 = c->a2; p1 = c->a3; }
+#define LRMD_UPD(M, K2, DR) \
+    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->N, part0(c), part1(c), c->S, kickA, kickB, d, js_ptr(c))
+    if (c->model == LRMD_RING) {
+        if (!drift) LRMD_UPD(1, false, false);
+        else if (kick2) LRMD_UPD(1, true, true);
+        else LRMD_UPD(1, false, true);
+    } else {
+        if (!drift) LRMD_UPD(2, false, false);
+        else if (kick2) LRMD_UPD(2, true, true);
+        else LRMD_UPD(2, false, true);
+    }
+#undef LRMD_UPD
+}
+
+void pair_ensure_force(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
+    if (!c->force_valid) { pair_force(L); c->force_valid = true; }
+}
+
+int pair_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
+    const Coef k = coefficients();
+    Launcher L{c, stream};
+    pair_ensure_force(L);
+    for (int64_t s = 0; s < n; ++s) {
+        pair_update(L, s > 0, true, k.B0 * dt, k.B0 * dt, k.D0 * dt);
+        pair_force(L);
+        pair_update(L, false, true, k.B1 * dt, 0.0, k.D1 * dt);
+        pair_force(L);
+        pair_update(L, false, true, k.B1 * dt, 0.0, k.D0 * dt);
+        pair_force(L);
+    }
+    pair_update(L, false, false, k.B0 * dt, 0.0, 0.0);
+    return L.rc;
+}
+
+bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
+
+}  // namespace
+
+// =========================================== C ABI =====================================================
+
+extern "C" {
+
+int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps) {
+    if (!out) return LRMD_EINVAL;
+    *out = nullptr;
+    if (model < LRMD_HMF || model > LRMD_GRAV2D || N < 1) return LRMD_EINVAL;
+    if (N > ((int64_t)1 << 40)) return LRMD_EINVAL;
+    if (model != LRMD_HMF && !finite_pos(eps)) return LRMD_EINVAL;
+    lrmd_ctx* c = new (std::nothrow) lrmd_ctx();
+    if (!c) return LRMD_EINVAL;
+    c->model = model;
+    c->N = N;
+    c->eps = (model == LRMD_HMF) ? 0.0 : eps;
+    resolve(c);
+    *out = c;
+    return LRMD_OK;
+}
+
+int lrmd_destroy(lrmd_ctx* c) {
+    if (!c) return LRMD_EINVAL;
+    drop_graph(c);
+    delete c;
+    return LRMD_OK;
+}
+
+int lrmd_workspace_bytes(const lrmd_ctx* c, size_t* bytes) {
+    if (!c || !bytes) return LRMD_EINVAL;
+    *bytes = c->lay.total;
+    return LRMD_OK;
+}
+
+int lrmd_set_workspace(lrmd_ctx* c, void* device_ptr, size_t bytes, void* cuda_stream) {
+    (void)cuda_stream;   // the workspace needs no initialisation: every buffer is written before it is read
+    if (!c || !device_ptr) return LRMD_EINVAL;
+    if (bytes < c->lay.total || ((uintptr_t)device_ptr % kAlign) != 0) return LRMD_EINVAL;
+    c->ws = static_cast<char*>(device_ptr);
+    c->force_valid = false;
+    c->js_valid = false;
+    drop_graph(c);
+    return LRMD_OK;
+}
+
+int lrmd_set_state(lrmd_ctx* c, double* a0, double* a1, double* a2, double* a3) {
+    if (!c || !a0 || !a1) return LRMD_EINVAL;
+    const bool two = c->model == LRMD_GRAV2D;
+    if (two ? (!a2 || !a3) : (a2 || a3)) return LRMD_EINVAL;
+    double* arr[4] = {a0, a1, a2, a3};
+    for (double* p : arr)
+        if (p && ((uintptr_t)p % 16) != 0) return LRMD_EINVAL;
+    // the HMF kernel uses 256-bit accesses on theta and p
+    if (c->model == LRMD_HMF && ((((uintptr_t)a0) % 32) != 0 || (((uintptr_t)a1) % 32) != 0)) return LRMD_EINVAL;
+    c->a0 = a0; c->a1 = a1; c->a2 = a2; c->a3 = a3;
+    c->state_set = true;
+    c->force_valid = false;
+    c->js_valid = false;
+    drop_graph(c);
+    return LRMD_OK;
+}
+
+static int ready(const lrmd_ctx* c) {
+    if (!c) return LRMD_EINVAL;
+    if (!c->state_set || !c->ws) return LRMD_ESTATE;
+    return LRMD_OK;
+}
+
+int lrmd_step(lrmd_ctx* c, int64_t n, double dt, void* cuda_stream) {
+    int rc = ready(c);
+    if (rc != LRMD_OK) return rc;
+    if (n < 0 || !std::isfinite(dt)) return LRMD_EINVAL;
+    if (n == 0) return LRMD_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    return c->model == LRMD_HMF ? hmf_step(c, n, dt, stream) : pair_step(c, n, dt, stream);
+}
+
+int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
+    int rc = ready(c);
+    if (rc != LRMD_OK) return rc;
+    if (!f0) return LRMD_EINVAL;
+    if (c->model == LRMD_GRAV2D ? !f1 : (f1 != nullptr)) return LRMD_EINVAL;
+    Launcher L{c, static_cast<cudaStream_t>(cuda_stream)};
+    if (c->model == LRMD_HMF) {
+        if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }
+        int64_t g = (c->N + kHmfThreads - 1) / kHmfThreads;
+        if (g > kHmfMaxGrid) g = kHmfMaxGrid;
+        L.go(hmf_force_kernel, dim3((unsigned)g), dim3(kHmfThreads), (const double*)c->a0, f0, c->N,
+             (const double2*)hmf_buf(c, c->cur), c->hmf_grid);
+    } else {
+        pair_ensure_force(L);
+        L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->N,
+             (const double*)part0(c), (const double*)part1(c), c->S, f0, f1);
+    }
+    return L.rc;
+}
+
+int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
+    int rc = ready(c);
+    if (rc != LRMD_OK) return rc;
+    if (!out4_device) return LRMD_EINVAL;
+    Launcher L{c, static_cast<cudaStream_t>(cuda_stream)};
+    const bool two = c->model == LRMD_GRAV2D;
+    const double* p0 = two ? c->a2 : c->a1;
+    const double* p1 = two ? c->a3 : nullptr;
+    int64_t gk = (c->N + kHmfThreads - 1) / kHmfThreads;
+    if (gk > kEnergyGrid) gk = kEnergyGrid;
+    L.go(kinetic_partial_kernel, dim3((unsigned)gk), dim3(kHmfThreads), p0, p1, c->N, kpart(c));
+    if (c->model == LRMD_HMF) {
+        if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }
+        L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
+             (const double2*)hmf_buf(c, c->cur), c->hmf_grid, (const double*)nullptr, 0, out4_device);
+    } else {
+        if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
+        const dim3 g((unsigned)c->itiles, (unsigned)c->S), b(kPairThreads);
+        // V = pre * sum_{i<j} t_ij = (pre/2) * sum_{i != j} t_ij
+        if (c->model == LRMD_RING)
+            L.go(pair_energy_kernel<1>, g, b, (const double2*)js_ptr(c), c->N, c->eps,
+                 -0.5 / (std::sqrt(2.0) * (double)c->N), vpart(c));
+        else
+            L.go(pair_energy_kernel<2>, g, b, (const double2*)js_ptr(c), c->N, c->eps, 0.5 / (double)c->N, vpart(c));
+        L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
+             (const double2*)nullptr, 0, (const double*)vpart(c), c->S * c->itiles, out4_device);
+    }
+    return L.rc;
+}
+
+int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
+    if (!c) return LRMD_EINVAL;
+    switch (key) {
+        case LRMD_OPT_PAIR_PRECISION:
+            if (value == 0) break;
+            if (value == 1) return LRMD_EUNSUPPORTED;   // fp32-pair variant: SURVEY.md 8(f) N1, not built yet
+            return LRMD_EINVAL;
+        case LRMD_OPT_JSPLIT:
+            if (value < 0 || value > 1024) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
+            c->opt_jsplit = value;
+            break;
+        case LRMD_OPT_GRAPH:
+            if (value < -1 || value > 1) return LRMD_EINVAL;
+            c->opt_graph = value;
+            break;
+        case LRMD_OPT_HMF_GRID:
+            if (value < 0 || value > kHmfMaxGrid) return LRMD_EINVAL;
+            if (c->model != LRMD_HMF && value != 0) return LRMD_EINVAL;
+            c->opt_hmf_grid = value;
+            break;
+        default:
+            return LRMD_EINVAL;
+    }
+    const size_t before = c->lay.total;
+    resolve(c);
+    drop_graph(c);
+    c->force_valid = false;
+    c->js_valid = false;
+    if (c->lay.total > before) c->ws = nullptr;   // back to "workspace not set"
+    return LRMD_OK;
+}
+
+int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
+    if (!c || !value) return LRMD_EINVAL;
+    switch (key) {
+        case LRMD_OPT_PAIR_PRECISION: *value = 0; break;
+        case LRMD_OPT_JSPLIT: *value = c->S; break;
+        case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
+        case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
+        default: return LRMD_EINVAL;
+    }
+    return LRMD_OK;
+}
+
+int lrmd_launch_count(const lrmd_ctx* c, int64_t* launches) {
+    if (!c || !launches) return LRMD_EINVAL;
+    *launches = c->launches;
+    return LRMD_OK;
+}
+
+int lrmd_last_cuda_error(const lrmd_ctx* c) { return c ? c->cuda_err : 0; }
+
+const char* lrmd_strerror(int code) {
+    switch (code) {
+        case LRMD_OK: return "ok";
+        case LRMD_EINVAL: return "invalid argument";
+        case LRMD_ESTATE: return "state or workspace not set";
+        case LRMD_ECUDA: return "CUDA error (see lrmd_last_cuda_error)";
+        case LRMD_EUNSUPPORTED: return "not implemented in this build";
+        default: return "unknown error code";
+    }
+}
+
+int lrmd_coefficients(double* out4_host) {
+    if (!out4_host) return LRMD_EINVAL;
+    const Coef k = coefficients();
+    out4_host[0] = k.B0; out4_host[1] = k.B1; out4_host[2] = k.D0; out4_host[3] = k.D1;
+    return LRMD_OK;
+}
+
+int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host) {
+    if (!x_host || !s_host || !c_host || n < 0) return LRMD_EINVAL;
+    for (int64_t i = 0; i < n; ++i) sincos_pi4(x_host[i], s_host[i], c_host[i]);
+    return LRMD_OK;
+}
+
+}  // extern "C"
