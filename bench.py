@@ -1,0 +1,404 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the lrmd hot path on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload KEY] [--only] [--impl reference]
+
+A bench "step" is one complete integrator time step of the workload (three force
+evaluations + the kick/drift updates — what the paper's Tables 1-3 time).  The primary workload is
+BASELINE.json configs[1] (Ring, N = 16,384, eps = 0.01, dt = 0.01); with one GPU and without --only
+the other single-GPU configs are measured too and reported under "others" in the same line.
+
+Numbers reported (all measured in this process, never under a profiler):
+  value      whole-job throughput, state resident in HBM, CUDA events on the launching stream
+  e2e        the same metric through lrmd_step_host: pinned HOST buffers, H2D + (3K+1) force
+             evaluations + D2H inside the timed region
+  roofline   the dominant kernel (pair-force kernel / HMF fused substage): algorithmic flops or bytes
+             per launch / its average launch duration (event pairs around every launch, second pass)
+  cpu_baseline  the oracle (oracle/lrmd_ref.cpp), as it stands, on this box's host cores, bounded sample
+
+Multi-GPU (torchrun, --gpus N): the path does not shard under BASELINE.json's north_star ("no sharding
+or collectives between GPUs"): N independent replicas, one per rank, weak scaling; value = units all
+ranks processed / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_BYTES = 126 * 1024 * 1024
+SM_COUNT = 148
+FP64_LANES_PER_SM = 64          # DFMA lanes per SM (guide: 148 SMs; FP64 issue = 64/clk/SM on B200)
+
+# flops per ordered pair with FMA = 2: Ring 7 DFMA + 5 DMUL = 19; 2D 7 DFMA + 2 DADD = 16
+PAIR_FLOP = {1: 19.0, 2: 16.0}
+PAIR_FP64_INSTR = {1: 12.0, 2: 9.0}
+HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` captures (profiles/*.md name the command); None = not captured yet.
+NCU_TRAFFIC_BYTES = {"ring_16k": None, "grav2d_64k": None, "hmf_5e7": None, "grav2d_1m": None, "hmf_1e4": None}
+
+DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+# ---- clocks sampler (nvidia-smi's numbers through NVML) ---------------------------------------------------
+
+class ClockSampler:
+    REASONS = {
+        0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+        0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+    }
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples, self.bits = [], 0
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nvml = None
+            return self
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def _run(self):
+        nv = self._nvml
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                get = getattr(nv, "nvmlDeviceGetCurrentClocksEventReasons", None) or nv.nvmlDeviceGetCurrentClocksThrottleReasons
+                self.bits |= int(get(self._h))
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join(timeout=2)
+        reasons = [name for bit, name in self.REASONS.items() if self.bits & bit]
+        return {
+            "sm_mhz": statistics.median(self.samples) if self.samples else None,
+            "sm_max_mhz": self.max_mhz,
+            "reasons": reasons,
+            "samples": len(self.samples),
+        }
+
+
+# ---- one workload on this rank's GPU ------------------------------------------------------------------------
+
+def units_per_force(w):
+    """(metric, unit, units per force evaluation)."""
+    if w.model == 0:
+        return "particle-steps/s", "particle-steps/s", None
+    return "pair-interactions/s", "pair-interactions/s", float(w.N) * float(w.N)
+
+
+def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
+    import torch
+    from paper_1212_0262_b200 import lrmd
+
+    dev = torch.device("cuda", torch.cuda.current_device())
+    peaks = measured_peaks()
+    st = w.state()
+    ctx = lrmd.Context(w.model, w.N, w.eps, device=dev)
+    ctx.set_state(*st)
+    stream = torch.cuda.current_stream(dev)
+    state_bytes = ctx.narrays * w.N * 8
+    larger_than_l2 = state_bytes > L2_BYTES
+    resident_by_design = w.key == "hmf_1e4"
+    flush = None
+    if not larger_than_l2 and not resident_by_design:
+        flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        if dist_ctx is not None:
+            dist_ctx.barrier()
+        torch.cuda.synchronize(dev)
+
+    def timed_pass(K):
+        """K steps; returns device ms (sum of the event pairs) on this rank."""
+        if flush is None:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx.step(K, w.dt)
+            b.record(stream)
+            b.synchronize()
+            return a.elapsed_time(b)
+        evs = []
+        for _ in range(K):
+            flush.fill_(1)                                   # untimed: outside the event pair
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx.step(1, w.dt)
+            b.record(stream)
+            evs.append((a, b))
+        torch.cuda.synchronize(dev)
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    # warm-up (also caches the force at the current positions)
+    timed_pass(W)
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device()).start()
+    l0 = ctx.launch_count()
+    ms = timed_pass(K)
+    launches = ctx.launch_count() - l0
+    barrier()
+    clocks = sampler.stop()
+    ms_max = ms
+    world = 1
+    if dist_ctx is not None:
+        import torch.distributed as dist
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_max = float(t.item())
+        world = dist.get_world_size()
+
+    metric, unit, upf = units_per_force(w)
+    if w.model == 0:
+        units_per_step = float(w.N)
+    else:
+        units_per_step = 3.0 * upf
+    value = world * units_per_step * K / (ms_max * 1e-3)
+
+    out = {
+        "metric": metric, "value": value, "unit": unit, "ms_per_step": ms_max / K,
+        "gpu_launches": int(launches), "clocks": clocks,
+        "l2": ("inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)) if larger_than_l2 else
+              ("not flushed: %.2f MB working set is on-chip by design, latency-bound case" % (state_bytes / 1e6)
+               if resident_by_design else "L2 flushed (256 MiB write) before every timed step"),
+        "options": {"jsplit": ctx.get_option(lrmd.OPT_JSPLIT), "graph": ctx.get_option(lrmd.OPT_GRAPH),
+                    "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID)},
+    }
+
+    # ---- roofline of the dominant kernel: second pass with an event pair around each of its launches
+    if with_roofline:
+        ctx.set_option(lrmd.OPT_KERNEL_TIMING, 1)
+        Kr = min(K, 2000)
+        ctx.kernel_time()
+        ms_r = timed_pass(Kr)
+        kms, kn = ctx.kernel_time()
+        ctx.set_option(lrmd.OPT_KERNEL_TIMING, 0)
+        avg_s = (kms / max(kn, 1)) * 1e-3
+        clk = (clocks.get("sm_mhz") or peaks["sm_max_mhz"])
+        if w.model == 0:
+            bytes_per_launch = HMF_BYTES_PER_PARTICLE_SUBSTAGE * w.N
+            achieved = bytes_per_launch / avg_s / 1e9
+            roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
+                    "algorithmic_bytes_per_launch": bytes_per_launch}
+        else:
+            flop = PAIR_FLOP[w.model] * w.N * w.N
+            achieved = flop / avg_s / 1e12
+            peak = SM_COUNT * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+            instr_rate = PAIR_FP64_INSTR[w.model] * w.N * w.N / avg_s
+            roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",
+                    "algorithmic_flop_per_launch": flop,
+                    "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
+                    "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
+        roof.update({"kernel": "hmf_substage_kernel" if w.model == 0 else "pair_force_kernel",
+                     "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
+                     "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
+                     "traffic": NCU_TRAFFIC_BYTES.get(w.key)})
+        out["roofline"] = roof
+
+    # ---- end to end through lrmd_step_host: pinned host buffers, copies inside the timed region
+    if with_e2e:
+        host = [torch.from_numpy(a.copy()).pin_memory() for a in st]
+        Ke = max(1, min(K, 20 if w.model != 0 else K))
+        ctx.step_host(host, 1, w.dt)                          # warm-up of the copy path
+        for h, a in zip(host, st):
+            h.copy_(torch.from_numpy(a))
+        barrier()
+        t0 = time.perf_counter()
+        ctx.step_host(host, Ke, w.dt)                         # synchronises the stream before returning
+        t1 = time.perf_counter()
+        dt_s = t1 - t0
+        if dist_ctx is not None:
+            import torch.distributed as dist
+            t = torch.tensor([dt_s], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt_s = float(t.item())
+        if w.model == 0:
+            e_units = float(w.N) * Ke
+        else:
+            e_units = (3.0 * Ke + 1.0) * upf
+        out["e2e"] = {"value": world * e_units / dt_s, "unit": unit, "h2d_bytes_per_step": state_bytes / Ke,
+                      "d2h_bytes_per_step": state_bytes / Ke, "steps_per_call": Ke,
+                      "note": "lrmd_step_host: H2D state + force evaluation + %d steps + D2H state, host wall clock "
+                              "around the synchronous call; bytes are per step of the %d-step call" % (Ke, Ke)}
+    ctx.close()
+    del flush
+    torch.cuda.empty_cache()
+    return out
+
+
+# ---- the oracle on the host cores --------------------------------------------------------------------------
+
+def oracle_sample_rate(w, seconds, nthreads=0):
+    """Times the oracle, as it stands, on a bounded sample of workload w for about `seconds`.
+    Returns (units_per_second, description, threads)."""
+    import numpy as np
+    from oracle import ref
+    threads = ref.max_threads() if nthreads <= 0 else nthreads
+    st = w.state()
+    if w.model == 0:
+        n_s = min(w.N, 2_000_000)
+        th, p = st[0][:n_s].copy(), st[1][:n_s].copy()
+        t0 = time.perf_counter()
+        f0, _ = ref.step(0, 0.0, th, None, p, None, 1, w.dt)
+        per_step = time.perf_counter() - t0
+        n = max(1, int(seconds / max(per_step, 1e-6)))
+        t0 = time.perf_counter()
+        ref.step(0, 0.0, th, None, p, None, n, w.dt, f0, None, force_valid=True)
+        el = time.perf_counter() - t0
+        return n_s * n / el, f"{n} serial steps of the first {n_s} particles (eqs.(6)-(7) path)", 1
+    q0, q1 = (st[0], st[1]) if w.model == 2 else (st[0], None)
+    rng = np.random.default_rng(1)
+    form = 1
+    r0 = max(threads * 8, 64)
+    rows = rng.choice(w.N, min(r0, w.N), replace=False)
+    t0 = time.perf_counter()
+    ref.forces_rows(w.model, w.eps, q0, q1, rows, form=form, nthreads=nthreads)
+    el = time.perf_counter() - t0
+    rate = len(rows) * w.N / el
+    R = int(min(w.N, max(len(rows), seconds * rate / w.N)))
+    rows = rng.choice(w.N, R, replace=False)
+    t0 = time.perf_counter()
+    ref.forces_rows(w.model, w.eps, q0, q1, rows, form=form, nthreads=nthreads)
+    el = time.perf_counter() - t0
+    what = "eq.(9) precomputed sin/cos form" if w.model == 1 else "eq.(3) force, true division"
+    return R * w.N / el, f"forces on {R} sampled rows x all {w.N} j ({what}), OpenMP over rows", threads
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle timed on the host cores; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    metric, unit, _ = units_per_force(w)
+    per_step_s = 2.0
+    rates = []
+    desc, threads = "", 1
+    for k in range(args.warmup + args.steps):
+        r, desc, threads = oracle_sample_rate(w, per_step_s)
+        if k >= args.warmup:
+            rates.append(r)
+    value = len(rates) / sum(1.0 / r for r in rates)
+    line = {
+        "impl": "reference", "metric": metric, "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt},
+        "cpu_baseline": {"value": value, "unit": unit, "cores": threads, "kind": "oracle", "sample": "per step: " + desc},
+        "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--workload", default="ring_16k")
+    ap.add_argument("--only", action="store_true", help="primary workload only (no 'others', no cpu_baseline)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+
+    from paper_1212_0262_b200 import inputs
+    w = inputs.WORKLOADS[args.workload]
+    if args.impl == "reference":
+        args.steps = args.steps or 3
+        args.warmup = 1 if args.warmup is None else args.warmup
+        return run_reference(args, w)
+
+    K = args.steps or DEFAULT_STEPS[w.key]
+    W = max(3, args.warmup if args.warmup is not None else 3)
+
+    import torch
+    from paper_1212_0262_b200 import lrmd
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    lrmd.load()
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dist_ctx = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist_ctx = dist
+
+    res = run_workload(w, K, W, dist_ctx)
+    line = {
+        "metric": res["metric"], "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt,
+                   "step": "one 4th-order time step = 3 force evaluations + kick/drift updates (PAPER.md:54-63)",
+                   "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
+                   "l2": res["l2"], "options": res["options"]},
+        "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
+        "roofline": res.get("roofline"),
+    }
+
+    if world == 1 and not args.only:
+        others = {}
+        for key in ("grav2d_64k", "hmf_5e7", "grav2d_1m", "hmf_1e4"):
+            if key == w.key:
+                continue
+            ow = inputs.WORKLOADS[key]
+            r = run_workload(ow, DEFAULT_STEPS[key], 3, None, with_e2e=(key != "grav2d_1m"))
+            others[key] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options",
+                                              "clocks", "roofline", "e2e") if k in r}
+            others[key]["steps"] = DEFAULT_STEPS[key]
+        line["others"] = others
+        rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
+        line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        print(json.dumps(line))
+    if dist_ctx is not None:
+        dist_ctx.barrier()
+        dist_ctx.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

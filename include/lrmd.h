@@ -63,7 +63,11 @@ enum {
     LRMD_OPT_JSPLIT = 1,         /* pair models: number of j-chunks per i-tile (0 = choose from N)     */
     LRMD_OPT_GRAPH = 2,          /* 1 = lrmd_step replays a captured CUDA graph of one step (default
                                     for small N), 0 = plain launches, -1 = choose from N              */
-    LRMD_OPT_HMF_GRID = 3        /* HMF: number of CTAs of the fused substage kernel (0 = choose)      */
+    LRMD_OPT_HMF_GRID = 3,       /* HMF: number of CTAs of the fused substage kernel (0 = choose)      */
+    LRMD_OPT_KERNEL_TIMING = 4   /* 1 = bracket every launch of the model's dominant kernel (HMF: the fused
+                                    substage kernel; RING/GRAV2D: the pair-force kernel) with a CUDA event
+                                    pair on the launching stream; read with lrmd_kernel_time.  Turns CUDA-graph
+                                    replay off while set.  Measurement aid: results are unchanged.          */
 };
 
 /* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.
@@ -91,6 +95,13 @@ int lrmd_set_state(lrmd_ctx* ctx, double* a0, double* a1, double* a2, double* a3
 /* Advance n >= 0 full steps of size dt (may be negative) of eq.(4).  n = 0 is a no-op. */
 int lrmd_step(lrmd_ctx* ctx, int64_t n, double dt, void* cuda_stream);
 
+/* End-to-end variant with HOST buffers (pinned memory recommended), same NULL pattern as lrmd_set_state:
+ * copies h_* into the bound device state arrays (cudaMemcpyAsync on the stream; this invalidates the
+ * cached force), advances n steps, copies the state back into h_* and SYNCHRONISES the stream before
+ * returning.  The device state arrays must have been bound with lrmd_set_state. */
+int lrmd_step_host(lrmd_ctx* ctx, double* h_a0, double* h_a1, double* h_a2, double* h_a3, int64_t n, double dt,
+                   void* cuda_stream);
+
 /* Write the force at the current positions: f0 = f (HMF, RING; f1 must be NULL) or
  * (f0, f1) = (fx, fy) (GRAV2D).  Uses the cached force if valid, else evaluates and caches it. */
 int lrmd_forces(lrmd_ctx* ctx, double* f0, double* f1, void* cuda_stream);
@@ -110,6 +121,12 @@ int lrmd_get_option(const lrmd_ctx* ctx, int key, int64_t* value);
  * since creation: the caller's evidence that the CUDA path ran. */
 int lrmd_launch_count(const lrmd_ctx* ctx, int64_t* launches);
 
+/* With LRMD_OPT_KERNEL_TIMING on: waits for the recorded events, writes the summed device time (ms)
+ * of the dominant kernel's launches since the last call (or since the option was set) and their
+ * number to the two HOST pointers, and resets the accumulation.  At most 16384 launches are recorded
+ * between reads; later ones run untimed. */
+int lrmd_kernel_time(lrmd_ctx* ctx, double* ms_total_host, int64_t* launches_host);
+
 /* The cudaError_t (as int) of the last failed CUDA call on this context, 0 if none. */
 int lrmd_last_cuda_error(const lrmd_ctx* ctx);
 
@@ -118,6 +135,11 @@ const char* lrmd_strerror(int code);
 
 /* Yoshida coefficients used by lrmd_step: out4_host = {B0, B1, D0, D1} (HOST pointer). */
 int lrmd_coefficients(double* out4_host);
+
+/* Diagnostic (HOST pointers, runs on the CPU, no GPU needed): evaluates the library's own fp64
+ * sincos arithmetic (csrc/trig.cuh, the routine the HMF and Ring kernels inline) on n host values,
+ * so that its accuracy can be checked against a multiprecision reference without a GPU. */
+int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host);
 
 #ifdef __cplusplus
 }

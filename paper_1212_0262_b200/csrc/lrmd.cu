@@ -10,6 +10,7 @@
 #include <new>
 #include <tuple>
 #include <utility>
+#include <vector>
 
 #include "hmf_kernels.cuh"
 #include "pair_kernels.cuh"
@@ -22,6 +23,7 @@ constexpr int kNumSm = 148;                 // B200
 constexpr size_t kAlign = 256;
 constexpr int kEnergyGrid = kNumSm * 4;     // CTAs of the kinetic-energy partial kernel
 constexpr int kGraphSteps = 8;              // steady-state steps per replayed CUDA graph
+constexpr size_t kMaxTimedEvents = 1 << 15; // LRMD_OPT_KERNEL_TIMING: at most 16384 timed launches between reads
 
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
@@ -62,6 +64,10 @@ struct lrmd_ctx {
     // bookkeeping
     int64_t launches = 0;
     int cuda_err = 0;
+    // LRMD_OPT_KERNEL_TIMING: event pairs around the dominant kernel's launches
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;      // 2 per timed launch (start, stop), created on demand
+    size_t ev_used = 0;
 };
 
 namespace {
@@ -164,6 +170,26 @@ struct Launcher {
         }
     }
 
+    // The dominant kernel of the model: bracketed by CUDA events on the launching stream when
+    // LRMD_OPT_KERNEL_TIMING is on (never inside a graph).
+    template <typename... KA, typename... A>
+    void go_timed(void (*kernel)(KA...), dim3 grid, dim3 block, A... a) {
+        const bool t = c->timing && !graph && rc == LRMD_OK && c->ev_used + 2 <= kMaxTimedEvents;
+        if (t) {
+            while (c->ev.size() < c->ev_used + 2) {
+                cudaEvent_t e;
+                if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); go(kernel, grid, block, a...); return; }
+                c->ev.push_back(e);
+            }
+            cudaEventRecord(c->ev[c->ev_used], stream);
+        }
+        go(kernel, grid, block, a...);
+        if (t) {
+            cudaEventRecord(c->ev[c->ev_used + 1], stream);
+            c->ev_used += 2;
+        }
+    }
+
     template <typename T, size_t... I>
     static void fill(void** ptrs, T& vals, std::index_sequence<I...>) {
         ((ptrs[I] = (void*)&std::get<I>(vals)), ...);
@@ -197,10 +223,10 @@ void hmf_substage(Launcher& L, bool kick2, double kickA, double kickB, double dr
     const int nxt = (cur + 1) % 3;
     const dim3 g(c->hmf_grid), b(kHmfThreads);
     if (kick2)
-        L.go(hmf_substage_kernel<true, true, true, true>, g, b, c->a0, c->a1, c->N, kickA, kickB, drift,
+        L.go_timed(hmf_substage_kernel<true, true, true, true>, g, b, c->a0, c->a1, c->N, kickA, kickB, drift,
              hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
     else
-        L.go(hmf_substage_kernel<true, false, true, true>, g, b, c->a0, c->a1, c->N, kickA, 0.0, drift,
+        L.go_timed(hmf_substage_kernel<true, false, true, true>, g, b, c->a0, c->a1, c->N, kickA, 0.0, drift,
              hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
     cur = nxt;
 }
@@ -252,7 +278,7 @@ int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     hmf_one_step(L, k, dt, false, cur);     // cur returns to c->cur after 3 substages
     int64_t left = n - 1;
     if (L.rc != LRMD_OK) return L.rc;
-    if (c->use_graph && left >= kGraphSteps) {
+    if (c->use_graph && !c->timing && left >= kGraphSteps) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
         cudaStreamIsCapturing(stream, &cs);
         if (cs == cudaStreamCaptureStatusNone) {
@@ -286,10 +312,10 @@ void pair_force(Launcher& L) {
     lrmd_ctx* c = L.c;
     const dim3 g((unsigned)c->itiles, (unsigned)c->S), b(kPairThreads);
     if (c->model == LRMD_RING)
-        L.go(pair_force_kernel<1>, g, b, js_ptr(c), c->N, c->eps, -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N),
+        L.go_timed(pair_force_kernel<1>, g, b, js_ptr(c), c->N, c->eps, -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N),
              part0(c), part1(c));
     else
-        L.go(pair_force_kernel<2>, g, b, js_ptr(c), c->N, c->eps, -2.0 / (double)c->N, part0(c), part1(c));
+        L.go_timed(pair_force_kernel<2>, g, b, js_ptr(c), c->N, c->eps, -2.0 / (double)c->N, part0(c), part1(c));
 }
 
 void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB, double d) {
@@ -360,6 +386,7 @@ int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps) {
 int lrmd_destroy(lrmd_ctx* c) {
     if (!c) return LRMD_EINVAL;
     drop_graph(c);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;
     return LRMD_OK;
 }
@@ -411,6 +438,35 @@ int lrmd_step(lrmd_ctx* c, int64_t n, double dt, void* cuda_stream) {
     if (n == 0) return LRMD_OK;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     return c->model == LRMD_HMF ? hmf_step(c, n, dt, stream) : pair_step(c, n, dt, stream);
+}
+
+int lrmd_step_host(lrmd_ctx* c, double* h0, double* h1, double* h2, double* h3, int64_t n, double dt,
+                   void* cuda_stream) {
+    int rc = ready(c);
+    if (rc != LRMD_OK) return rc;
+    const bool two = c->model == LRMD_GRAV2D;
+    if (!h0 || !h1 || (two ? (!h2 || !h3) : (h2 || h3))) return LRMD_EINVAL;
+    if (n < 0 || !std::isfinite(dt)) return LRMD_EINVAL;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    double* host[4] = {h0, h1, h2, h3};
+    double* dev[4] = {c->a0, c->a1, c->a2, c->a3};
+    const size_t bytes = sizeof(double) * (size_t)c->N;
+    const int narr = two ? 4 : 2;
+    cudaError_t e = cudaSuccess;
+    for (int k = 0; k < narr && e == cudaSuccess; ++k)
+        e = cudaMemcpyAsync(dev[k], host[k], bytes, cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_ECUDA; }
+    c->force_valid = false;
+    c->js_valid = false;
+    if (n > 0) {
+        rc = c->model == LRMD_HMF ? hmf_step(c, n, dt, stream) : pair_step(c, n, dt, stream);
+        if (rc != LRMD_OK) return rc;
+    }
+    for (int k = 0; k < narr && e == cudaSuccess; ++k)
+        e = cudaMemcpyAsync(host[k], dev[k], bytes, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_ECUDA; }
+    return LRMD_OK;
 }
 
 int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
@@ -484,6 +540,11 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (c->model != LRMD_HMF && value != 0) return LRMD_EINVAL;
             c->opt_hmf_grid = value;
             break;
+        case LRMD_OPT_KERNEL_TIMING:
+            if (value != 0 && value != 1) return LRMD_EINVAL;
+            c->timing = value != 0;
+            c->ev_used = 0;
+            return LRMD_OK;
         default:
             return LRMD_EINVAL;
     }
@@ -503,6 +564,7 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
         case LRMD_OPT_JSPLIT: *value = c->S; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
+        case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;
         default: return LRMD_EINVAL;
     }
     return LRMD_OK;
@@ -511,6 +573,22 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
 int lrmd_launch_count(const lrmd_ctx* c, int64_t* launches) {
     if (!c || !launches) return LRMD_EINVAL;
     *launches = c->launches;
+    return LRMD_OK;
+}
+
+int lrmd_kernel_time(lrmd_ctx* c, double* ms_total_host, int64_t* launches_host) {
+    if (!c || !ms_total_host || !launches_host) return LRMD_EINVAL;
+    double total = 0.0;
+    for (size_t k = 0; k + 1 < c->ev_used; k += 2) {
+        cudaError_t e = cudaEventSynchronize(c->ev[k + 1]);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]);
+        if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); c->ev_used = 0; return LRMD_ECUDA; }
+        total += (double)ms;
+    }
+    *ms_total_host = total;
+    *launches_host = (int64_t)(c->ev_used / 2);
+    c->ev_used = 0;
     return LRMD_OK;
 }
 

@@ -1,0 +1,314 @@
+"""Thin Python binding of the C ABI in ``include/lrmd.h`` (``liblrmd.so``).
+
+Argument marshalling only: every step of the hot path (force evaluation, kick/drift updates,
+energy sums, integrator sequencing — PAPER.md:46-110) runs in the CUDA kernels behind the C ABI.
+PyTorch is used for device memory and streams, nothing else.  There is no CPU fallback: if the
+library cannot be built/loaded, or a call is made without a CUDA device, this module raises.
+
+Two layers:
+  * module functions ``lrmd_create`` ... ``lrmd_coefficients`` — same names and argument order as
+    the C calls, raw pointers as ints, return the C return code;
+  * ``Context`` — owns the torch tensors (state, workspace) and raises ``LrmdError`` on a non-zero code.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HMF, RING, GRAV2D = 0, 1, 2
+OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+OPT_PAIR_PRECISION, OPT_JSPLIT, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
+
+#: every symbol include/lrmd.h declares (tests check the library exports each of them)
+SYMBOLS = (
+    "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
+    "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
+    "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
+)
+
+_lib = None
+_vp, _i64, _dbl, _int = C.c_void_p, C.c_int64, C.c_double, C.c_int
+
+
+class LrmdError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda_error: int = 0):
+        self.code = code
+        self.cuda_error = cuda_error
+        msg = f"{what}: {strerror(code)} (code {code})"
+        if cuda_error:
+            msg += f", cudaError {cuda_error}"
+        super().__init__(msg)
+
+
+def library_path() -> str:
+    from . import build as _build
+    return _build.OUT
+
+
+def load(build_if_missing: bool = True):
+    """Load ``liblrmd.so`` (building it with nvcc first if missing or stale).  Raises on failure."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    from . import build as _build
+    path = _build.build() if build_if_missing else _build.OUT
+    if not os.path.exists(path):
+        raise RuntimeError(f"liblrmd.so not found at {path}: the CUDA library is required (no CPU fallback)")
+    lib = C.CDLL(path)
+    lib.lrmd_create.argtypes = [C.POINTER(_vp), _int, _i64, _dbl]
+    lib.lrmd_destroy.argtypes = [_vp]
+    lib.lrmd_workspace_bytes.argtypes = [_vp, C.POINTER(C.c_size_t)]
+    lib.lrmd_set_workspace.argtypes = [_vp, _vp, C.c_size_t, _vp]
+    lib.lrmd_set_state.argtypes = [_vp, _vp, _vp, _vp, _vp]
+    lib.lrmd_step.argtypes = [_vp, _i64, _dbl, _vp]
+    lib.lrmd_step_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _vp]
+    lib.lrmd_forces.argtypes = [_vp, _vp, _vp, _vp]
+    lib.lrmd_energy.argtypes = [_vp, _vp, _vp]
+    lib.lrmd_set_option.argtypes = [_vp, _int, _i64]
+    lib.lrmd_get_option.argtypes = [_vp, _int, C.POINTER(_i64)]
+    lib.lrmd_launch_count.argtypes = [_vp, C.POINTER(_i64)]
+    lib.lrmd_kernel_time.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_i64)]
+    lib.lrmd_last_cuda_error.argtypes = [_vp]
+    lib.lrmd_strerror.argtypes = [_int]
+    lib.lrmd_strerror.restype = C.c_char_p
+    lib.lrmd_coefficients.argtypes = [C.POINTER(_dbl)]
+    lib.lrmd_host_sincos.argtypes = [_vp, _i64, _vp, _vp]
+    for name in SYMBOLS:
+        if name != "lrmd_strerror":
+            getattr(lib, name).restype = _int
+    _lib = lib
+    return lib
+
+
+# ---- raw calls: same names as the C ABI ---------------------------------------------------------------
+
+def lrmd_create(model: int, N: int, eps: float):
+    """Returns (rc, ctx_handle)."""
+    h = _vp()
+    rc = load().lrmd_create(C.byref(h), int(model), int(N), float(eps))
+    return rc, h.value
+
+
+def lrmd_destroy(ctx):
+    return load().lrmd_destroy(ctx)
+
+
+def lrmd_workspace_bytes(ctx):
+    """Returns (rc, bytes)."""
+    n = C.c_size_t(0)
+    rc = load().lrmd_workspace_bytes(ctx, C.byref(n))
+    return rc, int(n.value)
+
+
+def lrmd_set_workspace(ctx, device_ptr: int, nbytes: int, stream: int = 0):
+    return load().lrmd_set_workspace(ctx, device_ptr, nbytes, stream)
+
+
+def lrmd_set_state(ctx, a0: int, a1: int, a2: int | None = None, a3: int | None = None):
+    return load().lrmd_set_state(ctx, a0, a1, a2, a3)
+
+
+def lrmd_step(ctx, n: int, dt: float, stream: int = 0):
+    return load().lrmd_step(ctx, int(n), float(dt), stream)
+
+
+def lrmd_step_host(ctx, h0: int, h1: int, h2: int | None, h3: int | None, n: int, dt: float, stream: int = 0):
+    return load().lrmd_step_host(ctx, h0, h1, h2, h3, int(n), float(dt), stream)
+
+
+def lrmd_forces(ctx, f0: int, f1: int | None = None, stream: int = 0):
+    return load().lrmd_forces(ctx, f0, f1, stream)
+
+
+def lrmd_energy(ctx, out4_device: int, stream: int = 0):
+    return load().lrmd_energy(ctx, out4_device, stream)
+
+
+def lrmd_set_option(ctx, key: int, value: int):
+    return load().lrmd_set_option(ctx, int(key), int(value))
+
+
+def lrmd_get_option(ctx, key: int):
+    """Returns (rc, value)."""
+    v = _i64(0)
+    rc = load().lrmd_get_option(ctx, int(key), C.byref(v))
+    return rc, int(v.value)
+
+
+def lrmd_launch_count(ctx):
+    """Returns (rc, launches)."""
+    v = _i64(0)
+    rc = load().lrmd_launch_count(ctx, C.byref(v))
+    return rc, int(v.value)
+
+
+def lrmd_kernel_time(ctx):
+    """Returns (rc, ms_total, launches)."""
+    ms, n = _dbl(0.0), _i64(0)
+    rc = load().lrmd_kernel_time(ctx, C.byref(ms), C.byref(n))
+    return rc, float(ms.value), int(n.value)
+
+
+def lrmd_last_cuda_error(ctx) -> int:
+    return load().lrmd_last_cuda_error(ctx)
+
+
+def strerror(code: int) -> str:
+    return load().lrmd_strerror(int(code)).decode()
+
+
+lrmd_strerror = strerror
+
+
+def lrmd_coefficients():
+    """(B0, B1, D0, D1) used by lrmd_step."""
+    out = (_dbl * 4)()
+    rc = load().lrmd_coefficients(out)
+    if rc != OK:
+        raise LrmdError(rc, "lrmd_coefficients")
+    return tuple(float(v) for v in out)
+
+
+def lrmd_host_sincos(x):
+    """Diagnostic: the library's own sincos arithmetic evaluated on the host.  numpy in, (sin, cos) out."""
+    import numpy as np
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    s = np.empty_like(x)
+    c = np.empty_like(x)
+    rc = load().lrmd_host_sincos(x.ctypes.data, x.size, s.ctypes.data, c.ctypes.data)
+    if rc != OK:
+        raise LrmdError(rc, "lrmd_host_sincos")
+    return s, c
+
+
+# ---- convenience object ---------------------------------------------------------------------------------
+
+class Context:
+    """One simulation context on one CUDA device.  Owns the state tensors and the workspace.
+
+    ``state`` is (theta, p) for HMF/RING or (x, y, px, py) for GRAV2D, as numpy arrays or torch
+    tensors; they are copied to fp64 device tensors which ``step`` updates in place.
+    """
+
+    def __init__(self, model: int, N: int, eps: float = 0.0, device="cuda:0", options: dict | None = None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1212_0262_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._torch = torch
+        self.device = torch.device(device)
+        self.model, self.N, self.eps = int(model), int(N), float(eps)
+        load()
+        with torch.cuda.device(self.device):
+            rc, self._h = lrmd_create(model, N, eps)
+        if rc != OK:
+            self._h = None
+            raise LrmdError(rc, "lrmd_create")
+        self._ws = None
+        self._state = None
+        self._host = None
+        for k, v in (options or {}).items():
+            self._chk(lrmd_set_option(self._h, k, v), "lrmd_set_option")
+        self._bind_workspace()
+
+    # -- helpers
+    def _chk(self, rc, what):
+        if rc != OK:
+            raise LrmdError(rc, what, lrmd_last_cuda_error(self._h) if self._h else 0)
+
+    def _stream(self, stream=None) -> int:
+        s = stream if stream is not None else self._torch.cuda.current_stream(self.device)
+        return int(s.cuda_stream)
+
+    def _bind_workspace(self):
+        torch = self._torch
+        rc, nbytes = lrmd_workspace_bytes(self._h)
+        self._chk(rc, "lrmd_workspace_bytes")
+        self._ws = torch.empty(max(nbytes, 256) + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        self._chk(lrmd_set_workspace(self._h, ptr, nbytes, self._stream()), "lrmd_set_workspace")
+
+    @property
+    def narrays(self) -> int:
+        return 4 if self.model == GRAV2D else 2
+
+    def set_option(self, key: int, value: int):
+        self._chk(lrmd_set_option(self._h, key, value), "lrmd_set_option")
+        if key != OPT_KERNEL_TIMING:          # the others may change the workspace size
+            self._bind_workspace()
+
+    def get_option(self, key: int) -> int:
+        rc, v = lrmd_get_option(self._h, key)
+        self._chk(rc, "lrmd_get_option")
+        return v
+
+    def set_state(self, *arrays):
+        torch = self._torch
+        if len(arrays) != self.narrays:
+            raise ValueError(f"model {self.model} takes {self.narrays} state arrays")
+        st = []
+        for a in arrays:
+            t = torch.as_tensor(a, dtype=torch.float64)
+            if t.numel() != self.N:
+                raise ValueError("state arrays must have length N")
+            st.append(t.to(self.device, copy=True).contiguous())
+        self._state = st
+        ptrs = [t.data_ptr() for t in st] + [None] * (4 - len(st))
+        self._chk(lrmd_set_state(self._h, *ptrs), "lrmd_set_state")
+
+    @property
+    def state(self):
+        """The device tensors, updated in place by ``step``."""
+        return tuple(self._state)
+
+    def state_numpy(self):
+        return tuple(t.cpu().numpy() for t in self._state)
+
+    def step(self, n: int, dt: float, stream=None):
+        with self._torch.cuda.device(self.device):
+            self._chk(lrmd_step(self._h, n, dt, self._stream(stream)), "lrmd_step")
+
+    def step_host(self, host_arrays, n: int, dt: float, stream=None):
+        """End to end through ``lrmd_step_host``: ``host_arrays`` are (pinned) CPU fp64 tensors,
+        read as the initial state and overwritten with the final one."""
+        ptrs = [t.data_ptr() for t in host_arrays] + [None] * (4 - len(host_arrays))
+        with self._torch.cuda.device(self.device):
+            self._chk(lrmd_step_host(self._h, *ptrs, n, dt, self._stream(stream)), "lrmd_step_host")
+
+    def forces(self, stream=None):
+        torch = self._torch
+        f0 = torch.empty(self.N, dtype=torch.float64, device=self.device)
+        f1 = torch.empty(self.N, dtype=torch.float64, device=self.device) if self.model == GRAV2D else None
+        with torch.cuda.device(self.device):
+            self._chk(lrmd_forces(self._h, f0.data_ptr(), None if f1 is None else f1.data_ptr(),
+                                  self._stream(stream)), "lrmd_forces")
+        return (f0, f1) if f1 is not None else f0
+
+    def energy(self, stream=None):
+        """Device tensor {K, V, a, b} (see lrmd_energy)."""
+        torch = self._torch
+        out = torch.empty(4, dtype=torch.float64, device=self.device)
+        with torch.cuda.device(self.device):
+            self._chk(lrmd_energy(self._h, out.data_ptr(), self._stream(stream)), "lrmd_energy")
+        return out
+
+    def launch_count(self) -> int:
+        rc, v = lrmd_launch_count(self._h)
+        self._chk(rc, "lrmd_launch_count")
+        return v
+
+    def kernel_time(self):
+        """(ms_total, launches) of the dominant kernel since the last read (needs OPT_KERNEL_TIMING = 1)."""
+        rc, ms, n = lrmd_kernel_time(self._h)
+        self._chk(rc, "lrmd_kernel_time")
+        return ms, n
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lrmd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

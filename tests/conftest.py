@@ -18,3 +18,18 @@ def ref():
     from oracle import ref as _ref
     _ref.max_threads()
     return _ref
+
+
+@pytest.fixture(scope="session")
+def lrmd():
+    """The CUDA path's binding (paper_1212_0262_b200/lrmd.py); builds/loads liblrmd.so.
+    GPU tests fail (not skip) when the library or the device is missing: no silent fallback."""
+    from paper_1212_0262_b200 import lrmd as _lrmd
+    _lrmd.load()
+    return _lrmd
+
+
+@pytest.fixture(scope="session")
+def inputs():
+    from paper_1212_0262_b200 import inputs as _inputs
+    return _inputs

@@ -1,0 +1,143 @@
+"""Host-side checks of the C-ABI library (no GPU needed): it loads, exports every symbol
+include/lrmd.h declares, validates its arguments, resolves options, and its in-kernel sincos
+arithmetic (csrc/trig.cuh, run on the host through lrmd_host_sincos) is accurate to ~1 ulp
+against extended precision / mpmath (NOT against the oracle: the two share nothing)."""
+import ctypes as C
+import math
+import os
+import re
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HMF, RING, GRAV2D = 0, 1, 2
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "lrmd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(lrmd_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(lrmd):
+    lib = C.CDLL(lrmd.library_path())
+    declared = _declared_symbols()
+    assert len(declared) >= 14
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in include/lrmd.h but not exported"
+    assert set(declared) == set(lrmd.SYMBOLS)
+
+
+def test_create_validates_arguments(lrmd):
+    assert lrmd.lrmd_create(3, 10, 0.1)[0] == lrmd.EINVAL
+    assert lrmd.lrmd_create(-1, 10, 0.1)[0] == lrmd.EINVAL
+    assert lrmd.lrmd_create(HMF, 0, 0.0)[0] == lrmd.EINVAL
+    for eps in (0.0, -1.0, float("nan"), float("inf")):
+        assert lrmd.lrmd_create(RING, 10, eps)[0] == lrmd.EINVAL       # reading G6
+        assert lrmd.lrmd_create(GRAV2D, 10, eps)[0] == lrmd.EINVAL
+    rc, h = lrmd.lrmd_create(HMF, 10, float("nan"))                    # eps ignored for HMF
+    assert rc == lrmd.OK and h
+    assert lrmd.lrmd_destroy(h) == lrmd.OK
+    assert lrmd.lrmd_destroy(None) == lrmd.EINVAL
+
+
+def test_calls_before_state_and_workspace_are_estate(lrmd):
+    rc, h = lrmd.lrmd_create(RING, 1000, 0.01)
+    assert rc == lrmd.OK
+    assert lrmd.lrmd_step(h, 1, 0.1) == lrmd.ESTATE
+    assert lrmd.lrmd_forces(h, 256, None) == lrmd.ESTATE
+    assert lrmd.lrmd_energy(h, 256) == lrmd.ESTATE
+    assert lrmd.lrmd_step(None, 1, 0.1) == lrmd.EINVAL
+    # NULL pattern of set_state (pointers are never dereferenced on the host)
+    assert lrmd.lrmd_set_state(h, 4096, 8192, 4096, None) == lrmd.EINVAL
+    assert lrmd.lrmd_set_state(h, 4096, None) == lrmd.EINVAL
+    assert lrmd.lrmd_set_state(h, 4096 + 8, 8192) == lrmd.EINVAL      # misaligned
+    assert lrmd.lrmd_set_state(h, 4096, 8192) == lrmd.OK
+    assert lrmd.lrmd_step(h, 1, 0.1) == lrmd.ESTATE                    # workspace still missing
+    rc, nbytes = lrmd.lrmd_workspace_bytes(h)
+    assert rc == lrmd.OK and nbytes >= 1000 * 16 + 1000 * 8
+    assert lrmd.lrmd_set_workspace(h, 4096 + 16, nbytes) == lrmd.EINVAL  # not 256-aligned
+    assert lrmd.lrmd_set_workspace(h, 4096, nbytes - 1) == lrmd.EINVAL   # too small
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(GRAV2D, 1000, 1e-3)
+    assert lrmd.lrmd_set_state(h, 4096, 8192, None, None) == lrmd.EINVAL
+    assert lrmd.lrmd_set_state(h, 4096, 8192, 12288, 16384) == lrmd.OK
+    lrmd.lrmd_destroy(h)
+
+
+def test_options(lrmd):
+    rc, h = lrmd.lrmd_create(RING, 16384, 0.01)
+    rc, S = lrmd.lrmd_get_option(h, lrmd.OPT_JSPLIT)
+    assert rc == lrmd.OK and 1 <= S <= 64
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, 3) == lrmd.OK
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_JSPLIT) == (lrmd.OK, 3)
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, -2) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, 99, 0) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_HMF_GRID, 8) == lrmd.EINVAL   # not an HMF context
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 2) == lrmd.EINVAL
+    rc, b3 = lrmd.lrmd_workspace_bytes(h)
+    lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, 6)
+    rc, b6 = lrmd.lrmd_workspace_bytes(h)
+    assert b6 > b3                                     # partial-force rows grow with the j-split
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(HMF, 50_000_000, 0.0)
+    rc, g = lrmd.lrmd_get_option(h, lrmd.OPT_HMF_GRID)
+    assert rc == lrmd.OK and g % 148 == 0 and g >= 148   # whole waves of the 148 SMs
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(HMF, 5, 0.0)
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_HMF_GRID)[1] >= 1
+    lrmd.lrmd_destroy(h)
+
+
+def test_strerror_and_coefficients(lrmd):
+    assert lrmd.strerror(0) == "ok"
+    for code in (-1, -2, -3, -4, -77):
+        assert isinstance(lrmd.strerror(code), str) and lrmd.strerror(code)
+    B0, B1, D0, D1 = lrmd.lrmd_coefficients()
+    # Yoshida's order conditions (ref. [33] of the paper; reading G4), not the oracle's numbers
+    assert abs(2 * D0 + D1 - 1) < 1e-15 and abs(2 * (B0 + B1) - 1) < 1e-15
+    assert abs(2 * D0 ** 3 + D1 ** 3) < 1e-14
+    assert abs(B0 - D0 / 2) < 1e-16 and abs(B1 - (D0 + D1) / 2) < 1e-16
+
+
+def _ulp_err(got, exact_ld):
+    """|got - exact| in units of ulp(exact) (fp64), exact given in extended precision."""
+    e = np.asarray(exact_ld, dtype=np.longdouble)
+    ulp = np.spacing(np.abs(e).astype(np.float64)).astype(np.longdouble)
+    return np.abs(got.astype(np.longdouble) - e) / ulp
+
+
+@pytest.mark.parametrize("lo,hi", [(-0.8, 0.8), (-4.0, 4.0), (-100.0, 100.0), (-1e6, 1e6)])
+def test_kernel_sincos_accuracy_bulk(lrmd, lo, hi):
+    """x87 long double sin/cos (64-bit mantissa) as the reference on 200k points per range."""
+    if np.finfo(np.longdouble).nmant < 63:
+        pytest.skip("no extended-precision long double on this host")
+    rng = np.random.default_rng(17)
+    x = rng.uniform(lo, hi, 200_000)
+    s, c = lrmd.lrmd_host_sincos(x)
+    xl = x.astype(np.longdouble)
+    es, ec = _ulp_err(s, np.sin(xl)), _ulp_err(c, np.cos(xl))
+    # near zeros of sin/cos the error is bounded absolutely (2^-53 scale), not in ulps of the result
+    big_s, big_c = np.abs(s) > 1e-3, np.abs(c) > 1e-3
+    assert es[big_s].max() < 1.5 and ec[big_c].max() < 1.5
+    assert np.abs(s.astype(np.longdouble) - np.sin(xl)).max() < 2.5e-16
+    assert np.abs(c.astype(np.longdouble) - np.cos(xl)).max() < 2.5e-16
+    assert np.all(np.abs(s * s + c * c - 1) < 1e-15)
+
+
+def test_kernel_sincos_special_points_mpmath(lrmd):
+    mp.mp.dps = 40
+    pts = [0.0, -0.0, 1e-300, 1e-9, math.pi / 4, -math.pi / 4, math.pi / 2, math.pi, 3 * math.pi / 2, 2 * math.pi,
+           0.7853981633974484, 0.7853981633974482, 1.5, -1.5, 22.0, 355.0, 1e5 * math.pi, 2.0 ** 29, -(2.0 ** 29),
+           2.0 ** 30 - 1.0, 2.0 ** 30, 1e12, -1e15]
+    x = np.array(pts)
+    s, c = lrmd.lrmd_host_sincos(x)
+    for xi, si, ci in zip(pts, s, c):
+        es, ec = mp.sin(mp.mpf(xi)), mp.cos(mp.mpf(xi))
+        assert abs(mp.mpf(float(si)) - es) < mp.mpf(2) ** -52, (xi, si, es)
+        assert abs(mp.mpf(float(ci)) - ec) < mp.mpf(2) ** -52, (xi, ci, ec)
+    assert s[0] == 0.0 and c[0] == 1.0
+    sn, cn = lrmd.lrmd_host_sincos(np.array([float("nan"), float("inf")]))
+    assert np.all(np.isnan(sn)) and np.all(np.isnan(cn))

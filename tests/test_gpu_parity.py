@@ -1,0 +1,477 @@
+"""Parity of the CUDA path (through the C ABI, include/lrmd.h) with the oracle (oracle/lrmd_ref.cpp)
+on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+    forces      |f_gpu - f_ref|_i <= 1e-12 * A_i,  A_i = sum_{j != i} |f_ij|
+    trajectory  positions and momenta within 1e-9 (absolute) after 10 steps
+    energies    K, V within 1e-12 * sum |terms|        (proposed addition)
+    long run    max relative energy error of the same order of magnitude as the oracle's
+Several summation orders are correct (reading G15): the GPU result is additionally required to be
+bitwise reproducible run to run.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+HMF, RING, GRAV2D = 0, 1, 2
+FTOL = 1e-12
+XTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as _torch
+    assert _torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return _torch
+
+
+def _state(model, N, seed):
+    rng = np.random.default_rng(seed)
+    if model == GRAV2D:
+        u1, u2 = rng.random(N), rng.random(N)
+        r, ph = np.sqrt(u1), 2 * math.pi * u2
+        px, py = 0.1 * rng.standard_normal(N), 0.1 * rng.standard_normal(N)
+        return [r * np.cos(ph), r * np.sin(ph), px - px.mean(), py - py.mean()]
+    a = 1.5 if model == HMF else 1.0
+    return [rng.uniform(-a, a, N), rng.uniform(-0.5, 0.5, N)]
+
+
+def _eps(model):
+    return {HMF: 0.0, RING: 0.01, GRAV2D: 1e-3}[model]
+
+
+def _q(model, st):
+    return (st[0], st[1]) if model == GRAV2D else (st[0], None)
+
+
+def _p(model, st):
+    return (st[2], st[3]) if model == GRAV2D else (st[1], None)
+
+
+def _gpu_forces(lrmd, model, eps, st, options=None):
+    ctx = lrmd.Context(model, len(st[0]), eps, options=options)
+    ctx.set_state(*st)
+    f = ctx.forces()
+    out = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    n_launch = ctx.launch_count()
+    ctx.close()
+    assert n_launch > 0
+    return out
+
+
+def _check_forces(model, got, want, A):
+    for g, w, a in zip(got, want, A):
+        if g is None:
+            continue
+        err = np.abs(g - w)
+        # HMF goes through the identity eq.(6): its two O(1) products cos*My, sin*Mx cancel the self term
+        # only to rounding, so a floor of a few 2^-53 applies (matters only where A_i ~ 0, e.g. N = 1)
+        tol = FTOL * a + (4e-16 if model == HMF else 1e-300)
+        bad = np.nonzero(err > tol)[0]
+        assert bad.size == 0, (model, bad[:5], err[bad[:5]], tol[bad[:5]], float((err / tol).max()))
+
+
+# ---- forces: sizes that span several i-tiles / j-tiles, ragged tails, degenerate sizes ----------------
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 255, 256, 257, 511, 512, 513, 1000, 1024, 4099])
+def test_forces_match_oracle_small_and_ragged(lrmd, ref, torch, model, N):
+    eps = _eps(model)
+    st = _state(model, N, 1000 + N)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=(1 if model == HMF else 0))
+    got = _gpu_forces(lrmd, model, eps, st)
+    _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("S", [1, 2, 3, 7, 16])
+def test_forces_any_jsplit(lrmd, ref, torch, model, S):
+    """The (i-tile x j-chunk) grid with partial-force rows summed in index order (row a-U1)."""
+    eps = _eps(model)
+    N = 2500
+    st = _state(model, N, 77)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_JSPLIT: S})
+    _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+@pytest.mark.parametrize("grid", [1, 3, 148, 1184])
+def test_hmf_forces_any_grid(lrmd, ref, torch, grid):
+    N = 100_003
+    st = _state(HMF, N, 5)
+    f0, _, S0, _ = ref.forces_abs(HMF, 0.0, st[0], None, form=0)   # S_i >= A_i (O(N) bound)
+    got = _gpu_forces(lrmd, HMF, 0.0, st, options={lrmd.OPT_HMF_GRID: grid})
+    # at this N use the pair-sum-free bound: A_i is within a factor ~2 of S_i for a waterbag
+    assert np.all(np.abs(got[0] - f0) <= FTOL * 0.5 * S0)
+
+
+@pytest.mark.parametrize("model,eps", [(RING, 1e-3), (RING, 1.0), (RING, 1e4), (GRAV2D, 1e-6), (GRAV2D, 10.0)])
+def test_forces_other_softenings(lrmd, ref, torch, model, eps):
+    N = 1500
+    st = _state(model, N, 31)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    got = _gpu_forces(lrmd, model, eps, st)
+    if model == RING and eps < 0.01:
+        # eq.(9)'s denominator cancels to ~eps for close pairs: relative rounding 2^-53/eps per pair,
+        # x1.5 in d^(-3/2) (same allowance as the oracle's own eq.(8)-vs-eq.(9) pin)
+        A0 = A0 * max(1.0, 1.5 * 4e-16 / eps / FTOL)
+    _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+def test_forces_coincident_particles(lrmd, ref, torch):
+    """Degenerate input: pairs of particles at identical positions (d_ij = eps exactly)."""
+    for model in (RING, GRAV2D):
+        eps = _eps(model)
+        st = _state(model, 600, 3)
+        for a in st:
+            a[300:] = a[:300]
+        q0, q1 = _q(model, st)
+        f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+        got = _gpu_forces(lrmd, model, eps, st)
+        _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+# ---- the BASELINE.json configs at full size -----------------------------------------------------------
+
+def test_config1_hmf_1e4_forces_and_energy(lrmd, ref, torch, inputs):
+    w = inputs.WORKLOADS["hmf_1e4"]
+    th, p = w.state()
+    f_pair, _, A, _ = ref.forces_abs(HMF, 0.0, th, None, form=1)      # O(N^2) pair sum of eq.(2)
+    ctx = lrmd.Context(HMF, w.N)
+    ctx.set_state(th, p)
+    f = ctx.forces().cpu().numpy()
+    assert np.all(np.abs(f - f_pair) <= FTOL * A)
+    e = ctx.energy().cpu().numpy()
+    e_ref, e_abs = ref.energy(HMF, 0.0, th, None, p, None, form=0)
+    assert abs(e[0] - e_ref[0]) <= 1e-12 * e_abs[0] and abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
+    assert abs(e[2] - e_ref[2]) <= 1e-15 * 2 and abs(e[3] - e_ref[3]) <= 1e-15 * 2
+    ctx.close()
+
+
+@pytest.mark.parametrize("key", ["hmf_1e4", "ring_16k", "grav2d_64k"])
+def test_trajectory_10_steps_full_configs(lrmd, ref, torch, inputs, key):
+    """Configs 1-3 at full N: 10 steps, every position and momentum within 1e-9."""
+    w = inputs.WORKLOADS[key]
+    st = [a.copy() for a in w.state()]
+    ctx = lrmd.Context(w.model, w.N, w.eps)
+    ctx.set_state(*st)
+    ctx.step(10, w.dt)
+    got = ctx.state_numpy()
+    f_gpu = ctx.forces()
+    ctx.close()
+    q0, q1 = _q(w.model, st)
+    p0, p1 = _p(w.model, st)
+    rf0, rf1 = ref.step(w.model, w.eps, q0, q1, p0, p1, 10, w.dt, form=(0 if w.model == HMF else 1))
+    for g, r in zip(got, st):
+        assert np.max(np.abs(g - r)) <= XTOL
+    # the cached force after the step is f(q(t + 10 dt))
+    fg = f_gpu if w.model == GRAV2D else (f_gpu, None)
+    for g, r in zip(fg, (rf0, rf1)):
+        if g is not None:
+            assert np.max(np.abs(g.cpu().numpy() - r)) <= 1e-9 * max(1.0, np.max(np.abs(r)))
+
+
+def test_config2_ring_forces_and_energy_full(lrmd, ref, torch, inputs):
+    w = inputs.WORKLOADS["ring_16k"]
+    th, p = w.state()
+    f0, _, A0, _ = ref.forces_abs(RING, w.eps, th, None, form=0)
+    ctx = lrmd.Context(RING, w.N, w.eps)
+    ctx.set_state(th, p)
+    f = ctx.forces().cpu().numpy()
+    assert np.all(np.abs(f - f0) <= FTOL * A0)
+    e = ctx.energy().cpu().numpy()
+    e_ref, e_abs = ref.energy(RING, w.eps, th, None, p, None)
+    assert abs(e[0] - e_ref[0]) <= 1e-12 * e_abs[0]
+    assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
+    assert abs(e[2] - e_ref[2]) <= 1e-12 * np.sum(np.abs(p)) and e[3] == 0.0
+    ctx.close()
+
+
+def test_config3_grav2d_forces_and_energy_full(lrmd, ref, torch, inputs):
+    w = inputs.WORKLOADS["grav2d_64k"]
+    x, y, px, py = w.state()
+    rows = np.random.default_rng(9).choice(w.N, 2048, replace=False)
+    f0, f1, A0, A1 = ref.forces_rows(GRAV2D, w.eps, x, y, rows, with_abs=True)
+    ctx = lrmd.Context(GRAV2D, w.N, w.eps)
+    ctx.set_state(x, y, px, py)
+    fx, fy = (t.cpu().numpy() for t in ctx.forces())
+    assert np.all(np.abs(fx[rows] - f0) <= FTOL * A0) and np.all(np.abs(fy[rows] - f1) <= FTOL * A1)
+    e = ctx.energy().cpu().numpy()
+    e_ref, e_abs = ref.energy(GRAV2D, w.eps, x, y, px, py)
+    assert abs(e[0] - e_ref[0]) <= 1e-12 * e_abs[0]
+    assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
+    assert abs(e[2] - e_ref[2]) <= 1e-12 * np.sum(np.abs(px)) and abs(e[3] - e_ref[3]) <= 1e-12 * np.sum(np.abs(py))
+    ctx.close()
+
+
+def test_config4_hmf_5e7_sampled_and_invariants(lrmd, ref, torch, inputs):
+    """Config 4 at full size in bench.py's launch configuration: forces on all rows at t = 0 against
+    the oracle's eq.(6)-(7) path (tolerance scaled by the O(N) bound S_i >= A_i),
+    then 10 GPU steps and (i) forces at the GPU's final angles on sampled rows, (ii) energy and
+    momentum conservation, which hold at any size."""
+    w = inputs.WORKLOADS["hmf_5e7"]
+    th, p = w.state()
+    ctx = lrmd.Context(HMF, w.N)
+    ctx.set_state(th, p)
+    f = ctx.forces().cpu().numpy()
+    f_ref, _, S, _ = ref.forces_abs(HMF, 0.0, th, None, form=0)
+    assert np.all(np.abs(f - f_ref) <= FTOL * S)
+    e0 = ctx.energy().cpu().numpy()
+    e_ref, e_abs = ref.energy(HMF, 0.0, th, None, p, None, form=0)
+    assert abs(e0[0] - e_ref[0]) <= 1e-12 * e_abs[0] and abs(e0[1] - e_ref[1]) <= 1e-12 * e_abs[1]
+    P0 = float(ctx.state[1].sum())
+    ctx.step(10, w.dt)
+    e1 = ctx.energy().cpu().numpy()
+    thg, pg = ctx.state_numpy()
+    rows = np.random.default_rng(4).choice(w.N, 4096, replace=False)
+    fr, _, Sr, _ = ref.forces_rows(HMF, 0.0, thg, None, rows, with_abs=True)
+    fg = ctx.forces().cpu().numpy()
+    assert np.all(np.abs(fg[rows] - fr) <= FTOL * Sr)
+    E0, E1 = e0[0] + e0[1], e1[0] + e1[1]
+    assert abs((E1 - E0) / E0) < 1e-7                 # dt = 0.05, 4th order: ~1e-9 expected
+    assert abs(float(ctx.state[1].sum()) - P0) <= 1e-12 * float(np.sum(np.abs(pg)))
+    ctx.close()
+
+
+def test_config5_grav2d_1m_sampled_rows(lrmd, ref, torch, inputs):
+    """Config 5 at full size: forces on sampled rows (each against all N) at t = 0 and at the GPU's
+    positions after one step."""
+    w = inputs.WORKLOADS["grav2d_1m"]
+    x, y, px, py = w.state()
+    rows = np.random.default_rng(6).choice(w.N, 512, replace=False)
+    ctx = lrmd.Context(GRAV2D, w.N, w.eps)
+    ctx.set_state(x, y, px, py)
+    fx, fy = (t.cpu().numpy() for t in ctx.forces())
+    f0, f1, A0, A1 = ref.forces_rows(GRAV2D, w.eps, x, y, rows, with_abs=True)
+    assert np.all(np.abs(fx[rows] - f0) <= FTOL * A0) and np.all(np.abs(fy[rows] - f1) <= FTOL * A1)
+    assert abs(math.fsum(fx)) <= 1e-13 * math.fsum(np.abs(fx)) + 1e-12   # antisymmetry: total force 0
+    ctx.step(1, w.dt)
+    xg, yg, pxg, pyg = ctx.state_numpy()
+    fx, fy = (t.cpu().numpy() for t in ctx.forces())
+    f0, f1, A0, A1 = ref.forces_rows(GRAV2D, w.eps, xg, yg, rows, with_abs=True)
+    assert np.all(np.abs(fx[rows] - f0) <= FTOL * A0) and np.all(np.abs(fy[rows] - f1) <= FTOL * A1)
+    scale = math.fsum(np.abs(pxg))
+    assert abs(math.fsum(pxg)) <= 1e-12 * scale and abs(math.fsum(pyg)) <= 1e-12 * scale
+    ctx.close()
+
+
+# ---- energies ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+@pytest.mark.parametrize("N", [1, 2, 3, 513, 4099])
+def test_energy_matches_oracle(lrmd, ref, torch, model, N):
+    eps = _eps(model)
+    st = _state(model, N, 200 + N)
+    q0, q1 = _q(model, st)
+    p0, p1 = _p(model, st)
+    e_ref, e_abs = ref.energy(model, eps, q0, q1, p0, p1, form=(1 if model == HMF else 0))
+    ctx = lrmd.Context(model, N, eps)
+    ctx.set_state(*st)
+    e = ctx.energy().cpu().numpy()
+    ctx.close()
+    assert abs(e[0] - e_ref[0]) <= 1e-12 * e_abs[0] + 1e-300
+    assert abs(e[1] - e_ref[1]) <= 1e-12 * max(e_abs[1], 0.5 * N if model == HMF else 0.0) + 1e-300
+    assert abs(e[2] - e_ref[2]) <= 1e-12 * max(1.0, np.sum(np.abs(p0)))
+    assert abs(e[3] - e_ref[3]) <= 1e-12 * max(1.0, np.sum(np.abs(p1)) if p1 is not None else 1.0)
+
+
+@pytest.mark.parametrize("S", [1, 5])
+def test_energy_any_jsplit(lrmd, ref, torch, S):
+    for model in (RING, GRAV2D):
+        eps = _eps(model)
+        st = _state(model, 3000, 41)
+        q0, q1 = _q(model, st)
+        p0, p1 = _p(model, st)
+        e_ref, e_abs = ref.energy(model, eps, q0, q1, p0, p1)
+        ctx = lrmd.Context(model, 3000, eps, options={lrmd.OPT_JSPLIT: S})
+        ctx.set_state(*st)
+        e = ctx.energy().cpu().numpy()
+        ctx.close()
+        assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
+
+
+# ---- integrator properties on the GPU ---------------------------------------------------------------
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+def test_trajectory_small_ragged(lrmd, ref, torch, model):
+    eps = _eps(model)
+    N = 1337
+    st = _state(model, N, 12)
+    ctx = lrmd.Context(model, N, eps)
+    ctx.set_state(*st)
+    ctx.step(10, 0.01)
+    got = ctx.state_numpy()
+    ctx.close()
+    q0, q1 = _q(model, st)
+    p0, p1 = _p(model, st)
+    ref.step(model, eps, q0, q1, p0, p1, 10, 0.01, form=(0 if model == HMF else 1))
+    for g, r in zip(got, st):
+        assert np.max(np.abs(g - r)) <= XTOL
+
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+@pytest.mark.parametrize("graph", [0, 1])
+def test_n_steps_equals_n_single_steps_bitwise(lrmd, torch, model, graph):
+    """Force reuse (reading G3) and the merged closing+opening kick: step(n) == n x step(1), bit for bit;
+    with and without CUDA-graph replay."""
+    eps = _eps(model)
+    N = 3001
+    st = _state(model, N, 8)
+    a = lrmd.Context(model, N, eps, options={lrmd.OPT_GRAPH: graph})
+    a.set_state(*st)
+    a.step(20, 0.01)
+    b = lrmd.Context(model, N, eps, options={lrmd.OPT_GRAPH: 0})
+    b.set_state(*st)
+    for _ in range(20):
+        b.step(1, 0.01)
+    for x, y in zip(a.state_numpy(), b.state_numpy()):
+        assert np.array_equal(x, y)
+    a.close(); b.close()
+
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+def test_bitwise_reproducible_run_to_run(lrmd, torch, model):
+    eps = _eps(model)
+    N = 20_011
+    st = _state(model, N, 99)
+    outs = []
+    for _ in range(2):
+        ctx = lrmd.Context(model, N, eps)
+        ctx.set_state(*st)
+        ctx.step(3, 0.01)
+        e = ctx.energy().cpu().numpy()
+        outs.append(tuple(ctx.state_numpy()) + (e,))
+        ctx.close()
+    for x, y in zip(*outs):
+        assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+def test_time_reversibility_and_momentum_on_gpu(lrmd, torch, model):
+    """PAPER.md:52 'The approximation in eq. (4) is time reversible'; sum_i f_i = 0."""
+    eps = _eps(model)
+    N = 2048
+    st = _state(model, N, 15)
+    ctx = lrmd.Context(model, N, eps)
+    ctx.set_state(*st)
+    ctx.step(50, 0.01)
+    mid = ctx.state_numpy()
+    assert np.max(np.abs(mid[0] - st[0])) > 1e-3
+    pk = (2, 3) if model == GRAV2D else (1,)
+    scale = math.fsum(np.abs(mid[pk[0]]))
+    for k in pk:
+        assert abs(math.fsum(mid[k]) - math.fsum(st[k])) <= 1e-13 * scale
+    if model == GRAV2D:   # angular momentum
+        L0 = math.fsum(st[0] * st[3] - st[1] * st[2])
+        L1 = math.fsum(mid[0] * mid[3] - mid[1] * mid[2])
+        assert abs(L1 - L0) <= 1e-13 * scale
+    ctx.step(50, -0.01)
+    back = ctx.state_numpy()
+    ctx.close()
+    for g, r in zip(back, st):
+        assert np.max(np.abs(g - r)) < 1e-11
+
+
+def test_long_run_energy_error_same_order_as_oracle(lrmd, ref, torch, inputs):
+    """Config 1 in full (1,000 steps, N = 1e4): max_t |(E - E0)/E0| sampled every 50 steps, GPU vs oracle
+    ('of the same order of magnitude as for the CPU code')."""
+    w = inputs.WORKLOADS["hmf_1e4"]
+    th, p = w.state()
+    ctx = lrmd.Context(HMF, w.N)
+    ctx.set_state(th, p)
+    rth, rp = th.copy(), p.copy()
+    e = ctx.energy().cpu().numpy()
+    E0g = e[0] + e[1]
+    er, _ = ref.energy(HMF, 0.0, rth, None, rp, None)
+    E0r = er[0] + er[1]
+    worst_g = worst_r = 0.0
+    f0 = None
+    for k in range(w.steps // 50):
+        ctx.step(50, w.dt)
+        e = ctx.energy().cpu().numpy()
+        worst_g = max(worst_g, abs((e[0] + e[1] - E0g) / E0g))
+        f0, _ = ref.step(HMF, 0.0, rth, None, rp, None, 50, w.dt, f0, None, force_valid=(k > 0))
+        er, _ = ref.energy(HMF, 0.0, rth, None, rp, None)
+        worst_r = max(worst_r, abs((er[0] + er[1] - E0r) / E0r))
+    ctx.close()
+    assert worst_r > 0 and 0.1 <= worst_g / worst_r <= 10.0, (worst_g, worst_r)
+    assert worst_g < 1e-6
+
+
+@pytest.mark.parametrize("key,steps", [("ring_16k", 100), ("grav2d_64k", 50)])
+def test_pair_models_energy_error_level(lrmd, ref, torch, inputs, key, steps):
+    """Configs 2 and 3 in full on the GPU: the relative energy error over the whole run stays at the
+    4th-order level; the oracle's own error over the first 10 steps is of the same order."""
+    w = inputs.WORKLOADS[key]
+    st = w.state()
+    ctx = lrmd.Context(w.model, w.N, w.eps)
+    ctx.set_state(*st)
+    e = ctx.energy().cpu().numpy()
+    E0 = e[0] + e[1]
+    ctx.step(10, w.dt)
+    e = ctx.energy().cpu().numpy()
+    err10 = abs((e[0] + e[1] - E0) / E0)
+    ctx.step(steps - 10, w.dt)
+    e = ctx.energy().cpu().numpy()
+    err_end = abs((e[0] + e[1] - E0) / E0)
+    ctx.close()
+    rs = [a.copy() for a in st]
+    q0, q1 = _q(w.model, rs)
+    p0, p1 = _p(w.model, rs)
+    er0, _ = ref.energy(w.model, w.eps, q0, q1, p0, p1)
+    ref.step(w.model, w.eps, q0, q1, p0, p1, 10, w.dt, form=1)
+    er1, _ = ref.energy(w.model, w.eps, q0, q1, p0, p1)
+    ref10 = abs((er1[0] + er1[1] - er0[0] - er0[1]) / (er0[0] + er0[1]))
+    assert abs(E0 - (er0[0] + er0[1])) <= 1e-12 * abs(E0) * 10
+    assert err_end < 1e-5
+    assert max(err10, 1e-15) / max(ref10, 1e-15) < 10 and max(ref10, 1e-15) / max(err10, 1e-15) < 10
+
+
+# ---- the end-to-end entry point and error paths -------------------------------------------------------
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+def test_step_host_equals_step(lrmd, torch, model):
+    eps = _eps(model)
+    N = 5000
+    st = _state(model, N, 2)
+    a = lrmd.Context(model, N, eps)
+    a.set_state(*st)
+    a.step(4, 0.01)
+    b = lrmd.Context(model, N, eps)
+    b.set_state(*[np.zeros(N) for _ in st])
+    host = [torch.from_numpy(x.copy()).pin_memory() for x in st]
+    b.step_host(host, 4, 0.01)
+    for x, y in zip(a.state_numpy(), host):
+        assert np.array_equal(x, y.numpy())
+    a.close(); b.close()
+
+
+def test_set_state_invalidates_cached_force(lrmd, ref, torch):
+    N = 700
+    st = _state(RING, N, 1)
+    ctx = lrmd.Context(RING, N, 0.01)
+    ctx.set_state(*st)
+    f_a = ctx.forces().cpu().numpy()
+    st2 = _state(RING, N, 2)
+    ctx.set_state(*st2)
+    f_b = ctx.forces().cpu().numpy()
+    ctx.close()
+    want = ref.forces(RING, 0.01, st2[0], form=0)
+    assert np.max(np.abs(f_b - want)) < 1e-10 and np.max(np.abs(f_a - f_b)) > 1e-3
+
+
+def test_negative_n_and_nonfinite_dt_rejected(lrmd, torch):
+    ctx = lrmd.Context(HMF, 100)
+    ctx.set_state(*_state(HMF, 100, 0))
+    with pytest.raises(lrmd.LrmdError):
+        ctx.step(-1, 0.1)
+    with pytest.raises(lrmd.LrmdError):
+        ctx.step(1, float("nan"))
+    before = ctx.state_numpy()
+    ctx.step(0, 0.1)
+    assert all(np.array_equal(a, b) for a, b in zip(before, ctx.state_numpy()))
+    ctx.close()
