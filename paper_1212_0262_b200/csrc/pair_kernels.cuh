@@ -163,7 +163,7 @@ pair_force_kernel(const double2* __restrict__ js, long long N, double eps, doubl
                 if (i >= jbeg && i < jend) {   // remove the rounding-level j = i term again
                     double ny, y2;
                     ring_pair_parts(a[r], b[r], make_double2(a[r], b[r]), onepe, ny, y2);
-                    f0[r] = fma(-ny, y2, f0[r]);
+                    f0[r] -= __dmul_rn(ny, y2);   // the rounded product, so that N = 1 gives exactly 0
                 }
                 partial0[(long long)s * N + i] = pre * f0[r];
             } else {
