@@ -39,9 +39,9 @@ L2_BYTES = 126 * 1024 * 1024
 SM_COUNT = 148
 FP64_LANES_PER_SM = 64          # DFMA lanes per SM (guide: 148 SMs; FP64 issue = 64/clk/SM on B200)
 
-# flops per ordered pair with FMA = 2: Ring 7 DFMA + 5 DMUL = 19; 2D 7 DFMA + 2 DADD = 16
-PAIR_FLOP = {1: 19.0, 2: 16.0}
-PAIR_FP64_INSTR = {1: 12.0, 2: 9.0}
+# flops per ordered pair with FMA = 2: Ring 7 DFMA + 4 DMUL = 18; 2D 7 DFMA + 2 DADD = 16
+PAIR_FLOP = {1: 18.0, 2: 16.0}
+PAIR_FP64_INSTR = {1: 11.0, 2: 9.0}
 HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
@@ -196,8 +196,9 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
         "l2": ("inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)) if larger_than_l2 else
               ("not flushed: %.2f MB working set is on-chip by design, latency-bound case" % (state_bytes / 1e6)
                if resident_by_design else "L2 flushed (256 MiB write) before every timed step"),
-        "options": {"jsplit": ctx.get_option(lrmd.OPT_JSPLIT), "graph": ctx.get_option(lrmd.OPT_GRAPH),
-                    "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID)},
+        "options": {"pair_ctas": ctx.get_option(lrmd.OPT_PAIR_CTAS), "pair_variant": ctx.get_option(lrmd.OPT_PAIR_VARIANT),
+                    "pair_slots": ctx.get_option(lrmd.OPT_PAIR_SLOTS), "graph": ctx.get_option(lrmd.OPT_GRAPH),
+                    "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT)},
     }
 
     # ---- roofline of the dominant kernel: second pass with an event pair around each of its launches

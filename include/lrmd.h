@@ -60,14 +60,20 @@ enum {
 enum {
     LRMD_OPT_PAIR_PRECISION = 0, /* 0 = fp64 pair arithmetic (default); 1 = fp32 pair arithmetic with
                                     chunked fp32 -> fp64 accumulation (GRAV2D only)      */
-    LRMD_OPT_JSPLIT = 1,         /* pair models: number of j-chunks per i-tile (0 = choose from N)     */
+    LRMD_OPT_PAIR_CTAS = 1,      /* pair models: number of CTAs G the flattened (i-tile, j) space is divided
+                                    into, equal shares (0 = choose from N: 148 x resident CTAs x waves)  */
     LRMD_OPT_GRAPH = 2,          /* 1 = lrmd_step replays a captured CUDA graph of one step (default
                                     for small N), 0 = plain launches, -1 = choose from N              */
     LRMD_OPT_HMF_GRID = 3,       /* HMF: number of CTAs of the fused substage kernel (0 = choose)      */
-    LRMD_OPT_KERNEL_TIMING = 4   /* 1 = bracket every launch of the model's dominant kernel (HMF: the fused
+    LRMD_OPT_KERNEL_TIMING = 4,  /* 1 = bracket every launch of the model's dominant kernel (HMF: the fused
                                     substage kernel; RING/GRAV2D: the pair-force kernel) with a CUDA event
                                     pair on the launching stream; read with lrmd_kernel_time.  Turns CUDA-graph
                                     replay off while set.  Measurement aid: results are unchanged.          */
+    LRMD_OPT_HMF_VARIANT = 5,    /* HMF: launch shape of the fused substage kernel: 0 = register-prefetch
+                                    kernel, >= 1 = TMA-staged kernel shapes (-1 = choose from N)              */
+    LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
+                                    of the pair kernels (-1 = choose)                                          */
+    LRMD_OPT_PAIR_SLOTS = 7      /* read-only (lrmd_get_option): partial force rows per particle          */
 };
 
 /* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.
@@ -140,6 +146,14 @@ int lrmd_coefficients(double* out4_host);
  * sincos arithmetic (csrc/trig.cuh, the routine the HMF and Ring kernels inline) on n host values,
  * so that its accuracy can be checked against a multiprecision reference without a GPU. */
 int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host);
+
+/* Diagnostic (HOST pointers, runs on the CPU, no GPU needed): the work partition of the pair kernels
+ * (RING, GRAV2D) for the current options.  The N x N pair rectangle (every ordered pair is computed,
+ * PAPER.md:108; tiles after PAPER.md:100-106) is cut into i-tiles; the flattened (i-tile, j) space is
+ * divided into LRMD_OPT_PAIR_CTAS equal contiguous ranges, one per CTA.  Writes the segments of CTA
+ * `cta` as rows {tile, jbeg, jend, slot} (4 int64 each, at most max_seg rows) and their number to
+ * *nseg_host: the CTA adds the pairs (i in tile) x (jbeg <= j < jend) into partial force row `slot`. */
+int lrmd_pair_partition(const lrmd_ctx* ctx, int64_t cta, int64_t* seg4_host, int64_t max_seg, int64_t* nseg_host);
 
 #ifdef __cplusplus
 }

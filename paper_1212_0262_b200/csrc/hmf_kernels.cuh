@@ -126,6 +126,138 @@ hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long lon
     }
 }
 
+// ---- TMA-staged variant of the fused substage (large N) ------------------------------------------------
+// Same arithmetic per particle as hmf_substage_kernel, different data movement: a persistent CTA
+// per SM slot streams its chunks of theta and p through an NS-stage shared-memory ring.
+//   producer warp (one elected lane): 1-D TMA bulk loads global -> smem (mbarrier complete_tx),
+//       and, once the consumers are done with a stage, bulk stores smem -> global of the updated
+//       theta / p, then refills the stage as soon as the store has read it (wait_group.read);
+//   consumer warps: wait full[s], update their 4 particles of the chunk in place in shared memory,
+//       fence.proxy.async, one arrival per warp on done[s]; no CTA-wide barrier in the loop.
+// Bytes in flight per SM are set by NS x chunk (up to ~190 KB) instead of by registers per thread,
+// and both directions move as full-line bursts.  Chunk c goes to CTA c mod G (fixed), every
+// consumer thread adds its cos/sin terms in chunk order, block sums use fixed trees: deterministic.
+template <int CONSUMERS, int NS>
+struct HmfTma {
+    static constexpr int kChunk = 4 * CONSUMERS;            // particles per stage
+    static constexpr int kThreads = CONSUMERS + 32;         // + the producer warp
+    static constexpr size_t kSmemBytes = (size_t)NS * kChunk * 16 + 2 * NS * sizeof(uint64_t);
+};
+
+template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE, int CONSUMERS, int NS, int MINB>
+__global__ void __launch_bounds__(CONSUMERS + 32, MINB)
+hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double kickA, double kickB,
+                        double drift, const double2* __restrict__ partial_in, int g_in,
+                        double2* __restrict__ partial_out) {
+    using Cfg = HmfTma<CONSUMERS, NS>;
+    constexpr int C = Cfg::kChunk;
+    constexpr int T = Cfg::kThreads;
+    constexpr bool LOADP = KICK || DRIFT, STORE_TH = DRIFT, STORE_P = KICK, STORE = STORE_TH || STORE_P;
+    extern __shared__ __align__(128) unsigned char hmf_smem[];
+    double* sth = reinterpret_cast<double*>(hmf_smem);       // [NS][C]
+    double* sp = sth + (size_t)NS * C;                       // [NS][C]
+    uint64_t* full = reinterpret_cast<uint64_t*>(sp + (size_t)NS * C);
+    uint64_t* done = full + NS;
+    __shared__ double scratch[2 * (T / 32)];
+
+    const int tid = threadIdx.x;
+    const long long Nev = N & ~1LL;                          // bulk copies move multiples of 16 bytes
+    const long long nchunks = (Nev + C - 1) / C;
+    const long long first = blockIdx.x;
+    const int nmine = first < nchunks ? (int)((nchunks - 1 - first) / gridDim.x) + 1 : 0;
+
+    if (tid == CONSUMERS) {
+        for (int s = 0; s < NS; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&done[s], CONSUMERS / 32);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto chunk_base = [&](int k) { return (first + (long long)k * gridDim.x) * C; };
+    auto chunk_count = [&](long long i0) { return (int)((Nev - i0 < C) ? (Nev - i0) : C); };
+    auto issue_load = [&](int k) {
+        const int s = k % NS;
+        const long long i0 = chunk_base(k);
+        const uint32_t bytes = (uint32_t)chunk_count(i0) * 8u;
+        mbar_expect_tx(&full[s], LOADP ? 2u * bytes : bytes);
+        bulk_g2s(sth + (size_t)s * C, theta + i0, bytes, &full[s]);
+        if (LOADP) bulk_g2s(sp + (size_t)s * C, p + i0, bytes, &full[s]);
+    };
+    // the first NS chunks are in flight before the (latency-bound) magnetisation prologue
+    if (tid == CONSUMERS)
+        for (int k = 0; k < NS && k < nmine; ++k) issue_load(k);
+
+    double Mx = 0.0, My = 0.0;
+    if (KICK) hmf_magnetisation<T>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+
+    double accC = 0.0, accS = 0.0;
+    if (tid >= CONSUMERS) {
+        if (tid == CONSUMERS) {
+            for (int k = 0; k < nmine; ++k) {
+                const int s = k % NS;
+                mbar_wait(&done[s], (uint32_t)((k / NS) & 1));
+                if (STORE) {
+                    const long long i0 = chunk_base(k);
+                    const uint32_t bytes = (uint32_t)chunk_count(i0) * 8u;
+                    if (STORE_TH) bulk_s2g(theta + i0, sth + (size_t)s * C, bytes);
+                    if (STORE_P) bulk_s2g(p + i0, sp + (size_t)s * C, bytes);
+                    bulk_commit();
+                }
+                if (k + NS < nmine) {
+                    if (STORE) bulk_wait_read<0>();   // the store has read stage s: it may be overwritten
+                    issue_load(k + NS);
+                }
+            }
+            if (STORE) bulk_wait<0>();
+        }
+        __syncwarp();
+    } else {
+        for (int k = 0; k < nmine; ++k) {
+            const int s = k % NS;
+            const int cnt = chunk_count(chunk_base(k));
+            double2* t2 = reinterpret_cast<double2*>(sth + (size_t)s * C);
+            double2* p2 = reinterpret_cast<double2*>(sp + (size_t)s * C);
+            mbar_wait(&full[s], (uint32_t)((k / NS) & 1));
+            // 16-byte units tid and tid + CONSUMERS of the chunk (conflict-free LDS.128 / STS.128)
+            const int u0 = tid, u1 = tid + CONSUMERS;
+            const bool h0 = 2 * u0 < cnt, h1 = 2 * u1 < cnt;
+            double2 ta = make_double2(0.0, 0.0), tb = ta, pa = ta, pb = ta;
+            if (h0) { ta = t2[u0]; if (LOADP) pa = p2[u0]; }
+            if (h1) { tb = t2[u1]; if (LOADP) pb = p2[u1]; }
+            if (h0) {
+                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(ta.x, pa.x, Mx, My, kickA, kickB, drift, accC, accS);
+                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(ta.y, pa.y, Mx, My, kickA, kickB, drift, accC, accS);
+            }
+            if (h1) {
+                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(tb.x, pb.x, Mx, My, kickA, kickB, drift, accC, accS);
+                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(tb.y, pb.y, Mx, My, kickA, kickB, drift, accC, accS);
+            }
+            if (STORE) {
+                if (h0) { if (STORE_TH) t2[u0] = ta; if (STORE_P) p2[u0] = pa; }
+                if (h1) { if (STORE_TH) t2[u1] = tb; if (STORE_P) p2[u1] = pb; }
+                fence_proxy_async_smem();
+            }
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&done[s]);
+        }
+        // odd N: the last particle does not fit a 16-byte unit
+        if (blockIdx.x == 0 && tid == 0 && (N & 1)) {
+            const long long i = N - 1;
+            double th = theta[i], pp = LOADP ? p[i] : 0.0;
+            hmf_particle<KICK, KICK2, DRIFT, REDUCE>(th, pp, Mx, My, kickA, kickB, drift, accC, accS);
+            if (STORE_TH) theta[i] = th;
+            if (STORE_P) p[i] = pp;
+        }
+    }
+    if (REDUCE) {
+        double r[2] = {accC, accS};
+        block_sum<T, 2>(r, scratch);
+        if (tid == 0) partial_out[blockIdx.x] = make_double2(r[0], r[1]);
+    }
+}
+
 // f_i = cos(theta_i) My - sin(theta_i) Mx  -> f   (lrmd_forces; eq.(6))
 __global__ void __launch_bounds__(kHmfThreads)
 hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long long N,

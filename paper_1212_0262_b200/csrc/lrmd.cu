@@ -30,10 +30,10 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
     size_t hmf_partial = 0;   // 3 rotating buffers of kHmfMaxGrid double2 (HMF)
     size_t js = 0;            // packed j-stream double2[N] (pair models)
-    size_t partial0 = 0;      // [S][N] partial forces
-    size_t partial1 = 0;      // [S][N] (GRAV2D)
+    size_t partial0 = 0;      // [slots][N] partial forces
+    size_t partial1 = 0;      // [slots][N] (GRAV2D)
     size_t kpart = 0;         // 3 * kEnergyGrid
-    size_t vpart = 0;         // S * itiles (pair models)
+    size_t vpart = 0;         // one per CTA of the pair-energy kernel
     size_t total = 0;
 };
 
@@ -44,9 +44,12 @@ struct lrmd_ctx {
     int64_t N = 0;
     double eps = 0.0;
     // options as set (0 / -1 = choose)
-    int64_t opt_precision = 0, opt_jsplit = 0, opt_graph = -1, opt_hmf_grid = 0;
+    int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
+    int64_t opt_hmf_variant = -1, opt_pair_variant = -1;
     // resolved
-    int S = 1, itiles = 0, hmf_grid = 0;
+    int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
+    int slots = 1;              // partial force rows per particle (pair models)
+    lrmd::PairPart part{};      // work partition of the pair kernels
     bool use_graph = false;
     Layout lay;
     // bindings
@@ -64,6 +67,7 @@ struct lrmd_ctx {
     // bookkeeping
     int64_t launches = 0;
     int cuda_err = 0;
+    std::vector<const void*> smem_ready;   // kernels whose dynamic shared-memory limit has been raised
     // LRMD_OPT_KERNEL_TIMING: event pairs around the dominant kernel's launches
     bool timing = false;
     std::vector<cudaEvent_t> ev;      // 2 per timed launch (start, stop), created on demand
@@ -74,23 +78,27 @@ namespace {
 
 // ---- option resolution -------------------------------------------------------------------------------
 
-int choose_jsplit(int64_t N, int itiles) {
-    // Fill the 148 x kPairCtasPerSm resident CTA slots in (nearly) whole waves; keep each j-chunk
-    // at least 1024 elements so the tile pipeline amortises its prologue.
-    const int64_t slots = (int64_t)kNumSm * kPairCtasPerSm;
-    int64_t smax = N / 1024;
-    if (smax < 1) smax = 1;
-    if (smax > 64) smax = 64;
-    int best = 1;
-    double best_eff = 0.0;
-    for (int64_t s = 1; s <= smax; ++s) {
-        const int64_t ctas = (int64_t)itiles * s;
-        const int64_t waves = (ctas + slots - 1) / slots;
-        const double eff = (double)ctas / (double)(waves * slots);
-        if (eff > best_eff + 1e-9) { best_eff = eff; best = (int)s; }
-        if (eff >= 0.97) break;
+// Launch shapes compiled in (chosen from sweeps on B200, profiles/r01_sweeps.md).
+// HMF: variant 0 is the register-prefetch kernel (best below ~1e6 particles, where the step is latency
+// bound), the others the TMA-staged kernel <consumer threads, stages, CTAs per SM>.
+struct HmfVariant { int consumers, stages, minb; };
+constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 3, 2}, {512, 4, 1}, {480, 3, 2}};
+constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
+constexpr int64_t kHmfTmaMinN = 1000000;
+
+// Pair kernels: <threads, i per thread, j per stage, CTAs per SM, j unroll>.
+using PairCfg0 = PairCfg<128, 4, 256, 4, 4>;   // Ring default (88 registers)
+using PairCfg1 = PairCfg<128, 8, 256, 2, 2>;   // 2D default: one LDS.128 per 8 pairs
+using PairCfg2 = PairCfg<256, 4, 256, 2, 4>;
+constexpr int kNumPairVariants = 3;
+
+template <typename F>
+void with_pair_cfg(int v, F f) {
+    switch (v) {
+        case 1: f(PairCfg1{}); break;
+        case 2: f(PairCfg2{}); break;
+        default: f(PairCfg0{}); break;
     }
-    return best;
 }
 
 void resolve(lrmd_ctx* c) {
@@ -98,24 +106,61 @@ void resolve(lrmd_ctx* c) {
     Layout L;
     size_t off = 0;
     if (c->model == LRMD_HMF) {
-        const int64_t nvec = N >> 2;
-        int64_t g = c->opt_hmf_grid > 0 ? c->opt_hmf_grid : (nvec + kHmfThreads - 1) / kHmfThreads;
+        c->hmf_variant = c->opt_hmf_variant >= 0 ? (int)c->opt_hmf_variant : (N >= kHmfTmaMinN ? 1 : 0);
+        const HmfVariant hv = kHmfVariants[c->hmf_variant];
+        int64_t g;
+        if (c->hmf_variant == 0) {
+            const int64_t nvec = N >> 2;
+            g = c->opt_hmf_grid > 0 ? c->opt_hmf_grid : (nvec + kHmfThreads - 1) / kHmfThreads;
+        } else {
+            const int64_t chunk = 4 * (int64_t)hv.consumers;
+            const int64_t nchunks = ((N & ~(int64_t)1) + chunk - 1) / chunk;
+            g = c->opt_hmf_grid > 0 ? c->opt_hmf_grid : (int64_t)kNumSm * hv.minb;
+            if (g > nchunks) g = nchunks;
+        }
         if (g < 1) g = 1;
         if (g > kHmfMaxGrid) g = kHmfMaxGrid;
         c->hmf_grid = (int)g;
-        c->S = 1;
-        c->itiles = 0;
+        c->slots = 1;
         L.hmf_partial = off; off = align_up(off + 3 * sizeof(double2) * kHmfMaxGrid);
         c->use_graph = c->opt_graph < 0 ? (N <= (1 << 20)) : (c->opt_graph != 0);
     } else {
-        c->itiles = (int)((N + kPairITile - 1) / kPairITile);
-        c->S = c->opt_jsplit > 0 ? (int)c->opt_jsplit : choose_jsplit(N, c->itiles);
-        if ((int64_t)c->S > N) c->S = (int)N;
+        c->pair_variant = c->opt_pair_variant >= 0 ? (int)c->opt_pair_variant : (c->model == LRMD_GRAV2D ? 1 : 0);
+        int itile = 0, minb = 0;
+        with_pair_cfg(c->pair_variant, [&](auto cfg) { itile = decltype(cfg)::ITILE; minb = decltype(cfg)::MINB; });
+        const int64_t itiles = (N + itile - 1) / itile;
+        const int64_t Lpos = itiles * N;                       // flattened (i-tile, j) positions
+        const int64_t slots_hw = (int64_t)kNumSm * minb;       // resident CTAs on the device
+        int64_t G;
+        if (c->opt_pair_ctas > 0) {
+            G = c->opt_pair_ctas;
+        } else {
+            // one wave of equal ranges for small N; for large N ranges of about max(64Ki, N/8) positions
+            // (whole waves), which bounds both the tail of the last wave and the partial rows per tile
+            int64_t qt = N / 8 > 65536 ? N / 8 : 65536;
+            int64_t waves = (Lpos + slots_hw * qt / 2) / (slots_hw * qt);
+            if (waves < 1) waves = 1;
+            G = slots_hw * waves;
+            const int64_t gmax = Lpos / 64 > 1 ? Lpos / 64 : 1;   // at least 64 j per CTA
+            if (G > gmax) G = gmax;
+        }
+        if (G > Lpos) G = Lpos;
+        if (G < 1) G = 1;
+        PairPart P;
+        P.N = N; P.G = (int)G; P.q = Lpos / G; P.r = Lpos % G; P.itile = itile;
+        c->part = P;
+        int64_t smax = 1;
+        for (int64_t t = 0; t < itiles; ++t) {
+            long long first, last;
+            part_tile_ctas(P, t, first, last);
+            if (last - first + 1 > smax) smax = last - first + 1;
+        }
+        c->slots = (int)smax;
         c->hmf_grid = 0;
         L.js = off; off = align_up(off + sizeof(double2) * (size_t)N);
-        L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->S);
-        if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->S); }
-        L.vpart = off; off = align_up(off + sizeof(double) * (size_t)c->S * c->itiles);
+        L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots);
+        if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots); }
+        L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
         c->use_graph = false;
     }
     L.kpart = off; off = align_up(off + sizeof(double) * 3 * kEnergyGrid);
@@ -139,10 +184,24 @@ struct Launcher {
     int64_t nodes = 0;
     int rc = LRMD_OK;
 
+    size_t smem = 0;                   // dynamic shared memory of the next launch (reset after it)
+
     template <typename... KA, typename... A>
     void go(void (*kernel)(KA...), dim3 grid, dim3 block, A... a) {
         static_assert(sizeof...(KA) == sizeof...(A), "argument count");
+        const size_t shmem = smem;
+        smem = 0;
         if (rc != LRMD_OK) return;
+        if (shmem > 48 * 1024) {
+            bool ready = false;
+            for (const void* k : c->smem_ready) ready = ready || k == (const void*)kernel;
+            if (!ready) {
+                const cudaError_t ea = cudaFuncSetAttribute((const void*)kernel,
+                                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+                if (ea != cudaSuccess) { c->cuda_err = (int)ea; rc = LRMD_ECUDA; (void)cudaGetLastError(); return; }
+                c->smem_ready.push_back((const void*)kernel);
+            }
+        }
         std::tuple<KA...> vals{static_cast<KA>(a)...};
         void* ptrs[sizeof...(KA)];
         fill(ptrs, vals, std::index_sequence_for<KA...>{});
@@ -153,14 +212,14 @@ struct Launcher {
             kp.func = (void*)kernel;
             kp.gridDim = grid;
             kp.blockDim = block;
-            kp.sharedMemBytes = 0;
+            kp.sharedMemBytes = (unsigned)shmem;
             kp.kernelParams = ptrs;
             cudaGraphNode_t node;
             e = cudaGraphAddKernelNode(&node, graph, last ? &last : nullptr, last ? 1 : 0, &kp);
             last = node;
             ++nodes;
         } else {
-            e = cudaLaunchKernel((const void*)kernel, grid, block, ptrs, 0, stream);
+            e = cudaLaunchKernel((const void*)kernel, grid, block, ptrs, shmem, stream);
             if (e == cudaSuccess) ++c->launches;
         }
         if (e != cudaSuccess) {
@@ -217,24 +276,45 @@ Coef coefficients() {
 
 // ---- HMF sequencing ----------------------------------------------------------------------------------
 
+// Launch the fused substage kernel of the context's variant with the given stage flags.
+template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
+void hmf_launch(Launcher& L, bool timed, double kickA, double kickB, double drift, int in_buf, int out_buf) {
+    lrmd_ctx* c = L.c;
+    const dim3 g(c->hmf_grid);
+    const double2* pin = hmf_buf(c, in_buf);
+    double2* pout = hmf_buf(c, out_buf);
+#define LRMD_HMF_GO(KERNEL, BLOCK)                                                                           \
+    do {                                                                                                     \
+        if (timed) L.go_timed(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, kickA, kickB, drift, pin, c->hmf_grid, pout); \
+        else L.go(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, kickA, kickB, drift, pin, c->hmf_grid, pout);     \
+    } while (0)
+#define LRMD_HMF_TMA(V, CONS, NS, MINB)                                                                      \
+    case V:                                                                                                  \
+        L.smem = HmfTma<CONS, NS>::kSmemBytes;                                                               \
+        LRMD_HMF_GO((hmf_substage_tma_kernel<KICK, KICK2, DRIFT, REDUCE, CONS, NS, MINB>), CONS + 32);       \
+        break
+    switch (c->hmf_variant) {
+        LRMD_HMF_TMA(1, 512, 3, 2);
+        LRMD_HMF_TMA(2, 512, 4, 1);
+        LRMD_HMF_TMA(3, 480, 3, 2);
+        default:
+            LRMD_HMF_GO((hmf_substage_kernel<KICK, KICK2, DRIFT, REDUCE>), kHmfThreads);
+            break;
+    }
+#undef LRMD_HMF_TMA
+#undef LRMD_HMF_GO
+}
+
 // One fused substage: [kick kickA (+kickB)] -> drift -> reduce into the next partial buffer.
 void hmf_substage(Launcher& L, bool kick2, double kickA, double kickB, double drift, int& cur) {
-    lrmd_ctx* c = L.c;
     const int nxt = (cur + 1) % 3;
-    const dim3 g(c->hmf_grid), b(kHmfThreads);
-    if (kick2)
-        L.go_timed(hmf_substage_kernel<true, true, true, true>, g, b, c->a0, c->a1, c->N, kickA, kickB, drift,
-             hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
-    else
-        L.go_timed(hmf_substage_kernel<true, false, true, true>, g, b, c->a0, c->a1, c->N, kickA, 0.0, drift,
-             hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, nxt));
+    if (kick2) hmf_launch<true, true, true, true>(L, true, kickA, kickB, drift, cur, nxt);
+    else hmf_launch<true, false, true, true>(L, true, kickA, 0.0, drift, cur, nxt);
     cur = nxt;
 }
 
 void hmf_reduce_only(Launcher& L) {
-    lrmd_ctx* c = L.c;
-    L.go(hmf_substage_kernel<false, false, false, true>, dim3(c->hmf_grid), dim3(kHmfThreads), c->a0, c->a1, c->N,
-         0.0, 0.0, 0.0, hmf_buf(c, c->cur), c->hmf_grid, hmf_buf(c, c->cur));
+    hmf_launch<false, false, false, true>(L, false, 0.0, 0.0, 0.0, L.c->cur, L.c->cur);
 }
 
 // One full step.  merged: the closing kick B0 dt of the previous step is folded into this
@@ -246,9 +326,7 @@ void hmf_one_step(Launcher& L, const Coef& k, double dt, bool merged, int& cur) 
 }
 
 void hmf_closing_kick(Launcher& L, const Coef& k, double dt, int cur) {
-    lrmd_ctx* c = L.c;
-    L.go(hmf_substage_kernel<true, false, false, false>, dim3(c->hmf_grid), dim3(kHmfThreads), c->a0, c->a1, c->N,
-         k.B0 * dt, 0.0, 0.0, hmf_buf(c, cur), c->hmf_grid, hmf_buf(c, cur));
+    hmf_launch<true, false, false, false>(L, false, k.B0 * dt, 0.0, 0.0, cur, cur);
 }
 
 int hmf_build_graph(lrmd_ctx* c, const Coef& k, double dt) {
@@ -310,12 +388,16 @@ void pair_pack(Launcher& L) {
 
 void pair_force(Launcher& L) {
     lrmd_ctx* c = L.c;
-    const dim3 g((unsigned)c->itiles, (unsigned)c->S), b(kPairThreads);
-    if (c->model == LRMD_RING)
-        L.go_timed(pair_force_kernel<1>, g, b, js_ptr(c), c->N, c->eps, -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N),
-             part0(c), part1(c));
-    else
-        L.go_timed(pair_force_kernel<2>, g, b, js_ptr(c), c->N, c->eps, -2.0 / (double)c->N, part0(c), part1(c));
+    with_pair_cfg(c->pair_variant, [&](auto cfg) {
+        using CFG = decltype(cfg);
+        const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
+        if (c->model == LRMD_RING)
+            L.go_timed(pair_force_kernel<1, CFG>, g, b, js_ptr(c), c->part, c->eps,
+                       -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N), part0(c), part1(c));
+        else
+            L.go_timed(pair_force_kernel<2, CFG>, g, b, js_ptr(c), c->part, c->eps, -2.0 / (double)c->N, part0(c),
+                       part1(c));
+    });
 }
 
 void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB, double d) {
@@ -324,7 +406,7 @@ void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB
     double *q0 = c->a0, *q1 = nullptr, *p0 = c->a1, *p1 = nullptr;
     if (c->model == LRMD_GRAV2D) { q1 = c->a1; p0 = c->a2; p1 = c->a3; }
 #define LRMD_UPD(M, K2, DR) \
-    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->N, part0(c), part1(c), c->S, kickA, kickB, d, js_ptr(c))
+    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, part0(c), part1(c), kickA, kickB, d, js_ptr(c))
     if (c->model == LRMD_RING) {
         if (!drift) LRMD_UPD(1, false, false);
         else if (kick2) LRMD_UPD(1, true, true);
@@ -372,6 +454,7 @@ int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps) {
     *out = nullptr;
     if (model < LRMD_HMF || model > LRMD_GRAV2D || N < 1) return LRMD_EINVAL;
     if (N > ((int64_t)1 << 40)) return LRMD_EINVAL;
+    if (model != LRMD_HMF && N > ((int64_t)1 << 28)) return LRMD_EINVAL;   // O(N^2) models: 7e16 pairs per force
     if (model != LRMD_HMF && !finite_pos(eps)) return LRMD_EINVAL;
     lrmd_ctx* c = new (std::nothrow) lrmd_ctx();
     if (!c) return LRMD_EINVAL;
@@ -483,8 +566,8 @@ int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
              (const double2*)hmf_buf(c, c->cur), c->hmf_grid);
     } else {
         pair_ensure_force(L);
-        L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->N,
-             (const double*)part0(c), (const double*)part1(c), c->S, f0, f1);
+        L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->part,
+             (const double*)part0(c), (const double*)part1(c), f0, f1);
     }
     return L.rc;
 }
@@ -506,15 +589,19 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
              (const double2*)hmf_buf(c, c->cur), c->hmf_grid, (const double*)nullptr, 0, out4_device);
     } else {
         if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
-        const dim3 g((unsigned)c->itiles, (unsigned)c->S), b(kPairThreads);
         // V = pre * sum_{i<j} t_ij = (pre/2) * sum_{i != j} t_ij
-        if (c->model == LRMD_RING)
-            L.go(pair_energy_kernel<1>, g, b, (const double2*)js_ptr(c), c->N, c->eps,
-                 -0.5 / (std::sqrt(2.0) * (double)c->N), vpart(c));
-        else
-            L.go(pair_energy_kernel<2>, g, b, (const double2*)js_ptr(c), c->N, c->eps, 0.5 / (double)c->N, vpart(c));
+        with_pair_cfg(c->pair_variant, [&](auto cfg) {
+            using CFG = decltype(cfg);
+            const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
+            if (c->model == LRMD_RING)
+                L.go(pair_energy_kernel<1, CFG>, g, b, (const double2*)js_ptr(c), c->part, c->eps,
+                     -0.5 / (std::sqrt(2.0) * (double)c->N), vpart(c));
+            else
+                L.go(pair_energy_kernel<2, CFG>, g, b, (const double2*)js_ptr(c), c->part, c->eps, 0.5 / (double)c->N,
+                     vpart(c));
+        });
         L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
-             (const double2*)nullptr, 0, (const double*)vpart(c), c->S * c->itiles, out4_device);
+             (const double2*)nullptr, 0, (const double*)vpart(c), c->part.G, out4_device);
     }
     return L.rc;
 }
@@ -526,10 +613,20 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (value == 0) break;
             if (value == 1) return LRMD_EUNSUPPORTED;   // fp32-pair variant: SURVEY.md 8(f) N1, not built yet
             return LRMD_EINVAL;
-        case LRMD_OPT_JSPLIT:
-            if (value < 0 || value > 1024) return LRMD_EINVAL;
+        case LRMD_OPT_PAIR_CTAS:
+            if (value < 0 || value > (1 << 24)) return LRMD_EINVAL;
             if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
-            c->opt_jsplit = value;
+            c->opt_pair_ctas = value;
+            break;
+        case LRMD_OPT_HMF_VARIANT:
+            if (value < -1 || value >= kNumHmfVariants) return LRMD_EINVAL;
+            if (c->model != LRMD_HMF && value > 0) return LRMD_EINVAL;
+            c->opt_hmf_variant = value;
+            break;
+        case LRMD_OPT_PAIR_VARIANT:
+            if (value < -1 || value >= kNumPairVariants) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
+            c->opt_pair_variant = value;
             break;
         case LRMD_OPT_GRAPH:
             if (value < -1 || value > 1) return LRMD_EINVAL;
@@ -561,7 +658,10 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
     if (!c || !value) return LRMD_EINVAL;
     switch (key) {
         case LRMD_OPT_PAIR_PRECISION: *value = 0; break;
-        case LRMD_OPT_JSPLIT: *value = c->S; break;
+        case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : c->part.G; break;
+        case LRMD_OPT_HMF_VARIANT: *value = c->hmf_variant; break;
+        case LRMD_OPT_PAIR_VARIANT: *value = c->pair_variant; break;
+        case LRMD_OPT_PAIR_SLOTS: *value = c->slots; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;
@@ -609,6 +709,23 @@ int lrmd_coefficients(double* out4_host) {
     if (!out4_host) return LRMD_EINVAL;
     const Coef k = coefficients();
     out4_host[0] = k.B0; out4_host[1] = k.B1; out4_host[2] = k.D0; out4_host[3] = k.D1;
+    return LRMD_OK;
+}
+
+int lrmd_pair_partition(const lrmd_ctx* c, int64_t cta, int64_t* seg4_host, int64_t max_seg, int64_t* nseg_host) {
+    if (!c || !nseg_host || c->model == LRMD_HMF || cta < 0 || cta >= c->part.G || max_seg < 0) return LRMD_EINVAL;
+    if (max_seg > 0 && !seg4_host) return LRMD_EINVAL;
+    int64_t n = 0;
+    for_each_segment(c->part, (long long)cta, [&](long long tile, long long jbeg, long long jend, int slot) {
+        if (n < max_seg) {
+            seg4_host[4 * n + 0] = tile;
+            seg4_host[4 * n + 1] = jbeg;
+            seg4_host[4 * n + 2] = jend;
+            seg4_host[4 * n + 3] = slot;
+        }
+        ++n;
+    });
+    *nseg_host = n;
     return LRMD_OK;
 }
 

@@ -10,11 +10,12 @@
 //   * the j-stream is a packed double2 array written by the update kernel, and tiles are brought
 //     in by 1-D TMA bulk copies (cp.async.bulk -> UBLKCP) into a 2-stage ring guarded by mbarriers,
 //     issued by one thread while the CTA computes on the other stage;
-//   * a 2-D grid (i-tile, j-chunk): N/ITILE alone does not fill 148 SMs for N = 16,384, so the j
-//     range is split into S chunks; each CTA writes a partial force row partial[s][i] and the
-//     update kernel adds the S partials in index order (deterministic, no atomics);
+//   * a balanced 1-D partition of the flattened (i-tile, j) space over 148 x MINB x waves CTAs
+//     (PairPart below): N/ITILE alone does not fill 148 SMs for N = 16,384; each CTA writes one
+//     partial force row per tile it touches and the update kernel adds a tile's partial rows in
+//     slot order (deterministic, no atomics);
 //   * MUFU.RCP64H / MUFU.RSQ64H seed (~2^-20) + one cubic fp64 correction instead of rsqrt():
-//     2D 9 FP64 instructions per pair (7 DFMA + 2 DADD), Ring 12 (7 DFMA + 5 DMUL).
+//     2D 9 FP64 instructions per pair (7 DFMA + 2 DADD), Ring 11 (7 DFMA + 4 DMUL).
 // The j = i pair is computed like any other (PAPER.md:105 loops over all k): for eps > 0 it
 // contributes exactly 0 in 2D (dx = dy = 0) and a rounding-level term in the Ring rewrite eq.(9)
 // (s_i c_i - c_i s_i evaluated with one FMA), which the epilogue removes again.
@@ -25,11 +26,42 @@
 
 namespace lrmd {
 
-constexpr int kPairThreads = 128;   // threads per CTA
-constexpr int kPairR = 4;           // i-particles per thread
-constexpr int kPairITile = kPairThreads * kPairR;
-constexpr int kPairTJ = 256;        // j-elements per smem stage (4 KB)
-constexpr int kPairCtasPerSm = 4;   // enforced by __launch_bounds__ (<= 128 registers)
+// Launch shape of the pair kernels: THREADS threads per CTA, R i-particles per thread (i-tile =
+// THREADS x R), TJ j-elements per shared-memory stage, MINB resident CTAs per SM (register cap),
+// UNROLL j-iterations unrolled in the inner loop.
+template <int THREADS_, int R_, int TJ_, int MINB_, int UNROLL_>
+struct PairCfg {
+    static constexpr int THREADS = THREADS_, R = R_, TJ = TJ_, MINB = MINB_, UNROLL = UNROLL_;
+    static constexpr int ITILE = THREADS_ * R_;
+};
+
+// Work partition.  The N x N pair rectangle is cut into i-tiles of ITILE rows; the (i-tile, j)
+// space is flattened to L = itiles x N positions (position = tile * N + j) and divided into G
+// contiguous ranges of equal length (the first r ranges hold q + 1 positions, the others q), one
+// per CTA.  With G = 148 x MINB x waves every CTA carries the same number of pairs whatever N is
+// (N = 16,384 does not fill 148 SMs with whole tiles: SURVEY.md hard part 3).  A CTA's range
+// crosses at most ceil(q / N) tile boundaries; for each tile it touches it writes one partial
+// force row partial[slot][i], slot = cta - (first CTA touching the tile), and the update kernel
+// adds a tile's slots in slot order: deterministic, no atomics.
+struct PairPart {
+    long long N;      // particles
+    long long q, r;   // range lengths: q + 1 for CTAs < r, q for the others (q >= 1)
+    int G;            // CTAs
+    int itile;        // rows per i-tile
+};
+__host__ __device__ __forceinline__ long long part_bound(const PairPart& P, long long k) {
+    return k * P.q + (k < P.r ? k : P.r);
+}
+__host__ __device__ __forceinline__ long long part_owner(const PairPart& P, long long pos) {
+    const long long big = P.r * (P.q + 1);
+    return pos < big ? pos / (P.q + 1) : P.r + (pos - big) / P.q;
+}
+// slots of tile t: CTAs first..last touch it
+__host__ __device__ __forceinline__ void part_tile_ctas(const PairPart& P, long long t, long long& first,
+                                                        long long& last) {
+    first = part_owner(P, t * P.N);
+    last = part_owner(P, (t + 1) * P.N - 1);
+}
 
 // ---- per-pair arithmetic ---------------------------------------------------------------------------
 
@@ -57,220 +89,271 @@ __device__ __forceinline__ double rsqrt_refined(double d) {
     return fma(ye, g, y0);
 }
 
-// Ring eq.(9): returns (num * y, y^2) with y = d^(-1/2); term = num y^3
-__device__ __forceinline__ void ring_pair_parts(double ci, double si, double2 q, double onepe, double& ny, double& y2) {
+// Ring eq.(9): the pair term num d^(-3/2) as a product c * p of
+//   c = num y0^3                      (y0 = MUFU seed of d^(-1/2), relative error ~2^-20)
+//   p = 1 + (3/2) e + (15/8) e^2      (e = 1 - d y0^2;  (1 - e)^(-3/2) = p + O(e^3), |e^3| < 2^-56)
+// 11 FP64 instructions per pair with the accumulating FMA (7 DFMA + 4 DMUL) + 1 MUFU.RSQ64H:
+// num 2, d 2, y0^2 1, e 1, num y0 1, (num y0) y0^2 1, p 2, accumulate 1.
+__device__ __forceinline__ void ring_pair_parts(double ci, double si, double2 q, double onepe, double& c, double& p) {
     const double num = fma(si, q.x, -(ci * q.y));          // s_i c_j - c_i s_j
     const double d = fma(-si, q.y, fma(-ci, q.x, onepe));  // 1 + eps - c_i c_j - s_i s_j
-    const double y = rsqrt_refined(d);
-    ny = num * y;
-    y2 = y * y;
+    const double y0 = rsqrt_seed(d);
+    const double b = y0 * y0;
+    const double e = fma(-d, b, 1.0);
+    const double a = num * y0;
+    c = a * b;
+    const double g = fma(1.875, e, 1.5);
+    p = fma(g, e, 1.0);
 }
 
 // ---- j-tile pipeline ----------------------------------------------------------------------------------
 
+template <int TJ>
 struct PairSmem {
-    alignas(128) double2 tile[2][kPairTJ];
+    alignas(128) double2 tile[2][TJ];
     alignas(8) uint64_t full[2];
 };
 
-// Calls body(tile_ptr, count, j0) for consecutive tiles of [jbeg, jend) of the packed j-stream.
-template <typename Body>
-__device__ __forceinline__ void for_each_jtile(PairSmem& sm, const double2* __restrict__ js, long long jbeg,
-                                               long long jend, Body body) {
-    const int ntiles = (int)((jend - jbeg + kPairTJ - 1) / kPairTJ);
-    if (threadIdx.x == 0) {
-        mbar_init(&sm.full[0], 1);
-        mbar_init(&sm.full[1], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
-    if (threadIdx.x == 0 && ntiles > 0) {
-        const long long c0 = (jend - jbeg < kPairTJ) ? (jend - jbeg) : kPairTJ;
-        mbar_expect_tx(&sm.full[0], (uint32_t)(c0 * sizeof(double2)));
-        bulk_g2s(sm.tile[0], js + jbeg, (uint32_t)(c0 * sizeof(double2)), &sm.full[0]);
-    }
-    uint32_t phase[2] = {0u, 0u};
-    for (int t = 0; t < ntiles; ++t) {
-        const int s = t & 1;
-        const long long j0 = jbeg + (long long)t * kPairTJ;
-        if (threadIdx.x == 0 && t + 1 < ntiles) {
-            // stage s^1 was consumed in iteration t-1; every thread passed the barrier that ended it
-            const long long j1 = j0 + kPairTJ;
-            const long long c1 = (jend - j1 < kPairTJ) ? (jend - j1) : kPairTJ;
-            mbar_expect_tx(&sm.full[s ^ 1], (uint32_t)(c1 * sizeof(double2)));
-            bulk_g2s(sm.tile[s ^ 1], js + j1, (uint32_t)(c1 * sizeof(double2)), &sm.full[s ^ 1]);
+// Two-stage ring of j-tiles filled by 1-D TMA bulk copies.  init() once per CTA; run() may be
+// called for several j-ranges in turn (every copy it issues is consumed before it returns, so the
+// barrier phases carry over).
+template <int TJ>
+struct JTilePipe {
+    PairSmem<TJ>& sm;
+    uint32_t phases = 0u;   // bit s = parity the next wait on stage s expects
+    __device__ __forceinline__ explicit JTilePipe(PairSmem<TJ>& s) : sm(s) {}
+    __device__ __forceinline__ void init() {
+        if (threadIdx.x == 0) {
+            mbar_init(&sm.full[0], 1);
+            mbar_init(&sm.full[1], 1);
+            mbar_fence_init();
         }
-        mbar_wait(&sm.full[s], phase[s]);
-        phase[s] ^= 1u;
-        const int cnt = (int)((jend - j0 < kPairTJ) ? (jend - j0) : kPairTJ);
-        body(sm.tile[s], cnt, j0);
         __syncthreads();
     }
-}
+    // Calls body(tile_ptr, count, j0) for consecutive tiles of [jbeg, jend) of the packed j-stream.
+    template <typename Body>
+    __device__ __forceinline__ void run(const double2* __restrict__ js, long long jbeg, long long jend, Body body) {
+        const int ntiles = (int)((jend - jbeg + TJ - 1) / TJ);
+        if (threadIdx.x == 0 && ntiles > 0) {
+            const long long c0 = (jend - jbeg < TJ) ? (jend - jbeg) : TJ;
+            mbar_expect_tx(&sm.full[0], (uint32_t)(c0 * sizeof(double2)));
+            bulk_g2s(sm.tile[0], js + jbeg, (uint32_t)(c0 * sizeof(double2)), &sm.full[0]);
+        }
+        for (int t = 0; t < ntiles; ++t) {
+            const int s = t & 1;
+            const long long j0 = jbeg + (long long)t * TJ;
+            if (threadIdx.x == 0 && t + 1 < ntiles) {
+                // stage s^1 was consumed in iteration t-1; every thread passed the barrier that ended it
+                const long long j1 = j0 + TJ;
+                const long long c1 = (jend - j1 < TJ) ? (jend - j1) : TJ;
+                mbar_expect_tx(&sm.full[s ^ 1], (uint32_t)(c1 * sizeof(double2)));
+                bulk_g2s(sm.tile[s ^ 1], js + j1, (uint32_t)(c1 * sizeof(double2)), &sm.full[s ^ 1]);
+            }
+            mbar_wait(&sm.full[s], (phases >> s) & 1u);
+            phases ^= 1u << s;
+            const int cnt = (int)((jend - j0 < TJ) ? (jend - j0) : TJ);
+            body(sm.tile[s], cnt, j0);
+            __syncthreads();
+        }
+    }
+};
 
-__device__ __forceinline__ void jchunk_bounds(long long N, int S, int s, long long& jbeg, long long& jend) {
-    jbeg = (N * (long long)s) / S;
-    jend = (N * (long long)(s + 1)) / S;
+// Calls seg(tile, jbeg, jend, slot) for every (i-tile, j-range) segment of CTA k's range.
+template <typename Seg>
+__host__ __device__ __forceinline__ void for_each_segment(const PairPart& P, long long k, Seg seg) {
+    long long pos = part_bound(P, k);
+    const long long end = part_bound(P, k + 1);
+    while (pos < end) {
+        const long long t = pos / P.N;
+        const long long jbeg = pos - t * P.N;
+        const long long jend = (end - pos < P.N - jbeg) ? jbeg + (end - pos) : P.N;
+        const int slot = (int)(k - part_owner(P, t * P.N));
+        seg(t, jbeg, jend, slot);
+        pos += jend - jbeg;
+    }
 }
 
 // ---- force kernels (rows a-P1r, a-P1g) --------------------------------------------------------------
 
-// grid = (ceil(N/ITILE), S).  partial0/1: [S][N] partial forces (with the model's prefactor).
-template <int MODEL>
-__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
-pair_force_kernel(const double2* __restrict__ js, long long N, double eps, double pre,
+// grid = P.G CTAs.  partial0/1: [slots][N] partial forces (with the model's prefactor).
+template <int MODEL, typename CFG>
+__global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
+pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double pre,
                   double* __restrict__ partial0, double* __restrict__ partial1) {
-    __shared__ PairSmem sm;
-    const long long ibase = (long long)blockIdx.x * kPairITile + threadIdx.x;
-    const int S = gridDim.y, s = blockIdx.y;
-    long long jbeg, jend;
-    jchunk_bounds(N, S, s, jbeg, jend);
-
-    double a[kPairR], b[kPairR], f0[kPairR], f1[kPairR];
-#pragma unroll
-    for (int r = 0; r < kPairR; ++r) {
-        const long long i = ibase + (long long)r * kPairThreads;
-        const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
-        a[r] = q.x;
-        b[r] = q.y;
-        f0[r] = 0.0;
-        f1[r] = 0.0;
-    }
+    constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
+    __shared__ PairSmem<TJ> sm;
+    JTilePipe<TJ> pipe(sm);
+    pipe.init();
+    const long long N = P.N;
     const double onepe = 1.0 + eps;
 
-    for_each_jtile(sm, js, jbeg, jend, [&](const double2* tile, int cnt, long long) {
-#pragma unroll 4
-        for (int jj = 0; jj < cnt; ++jj) {
-            const double2 q = tile[jj];   // broadcast LDS.128
+    for_each_segment(P, blockIdx.x, [&](long long tile, long long jbeg, long long jend, int slot) {
+        const long long ibase = tile * CFG::ITILE + threadIdx.x;
+        double a[R], b[R], f0[R], f1[R];
 #pragma unroll
-            for (int r = 0; r < kPairR; ++r) {
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
+            a[r] = q.x;
+            b[r] = q.y;
+            f0[r] = 0.0;
+            f1[r] = 0.0;
+        }
+        auto pair = [&](const double2 q) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
                 if (MODEL == 2) {
                     grav_pair(a[r], b[r], q, eps, f0[r], f1[r]);
                 } else {
-                    double ny, y2;
-                    ring_pair_parts(a[r], b[r], q, onepe, ny, y2);
-                    f0[r] = fma(ny, y2, f0[r]);
+                    double c, p;
+                    ring_pair_parts(a[r], b[r], q, onepe, c, p);
+                    f0[r] = fma(c, p, f0[r]);
+                }
+            }
+        };
+        pipe.run(js, jbeg, jend, [&](const double2* tl, int cnt, long long) {
+            if (cnt == TJ) {
+                // the next group's j-elements are loaded (broadcast LDS.128) before this group's arithmetic
+                constexpr int U = CFG::UNROLL;
+                double2 qn[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) qn[u] = tl[u];
+#pragma unroll 1
+                for (int jj = 0; jj < TJ; jj += U) {
+                    double2 q[U];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) q[u] = qn[u];
+                    const int nx = (jj + U < TJ) ? jj + U : 0;   // last group: harmless reload of group 0
+#pragma unroll
+                    for (int u = 0; u < U; ++u) qn[u] = tl[nx + u];
+#pragma unroll
+                    for (int u = 0; u < U; ++u) pair(q[u]);
+                }
+            } else {
+#pragma unroll 2
+                for (int jj = 0; jj < cnt; ++jj) pair(tl[jj]);
+            }
+        });
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            if (i < N) {
+                if (MODEL == 1) {
+                    if (i >= jbeg && i < jend) {   // remove the rounding-level j = i term again
+                        double c, p;
+                        ring_pair_parts(a[r], b[r], make_double2(a[r], b[r]), onepe, c, p);
+                        f0[r] -= __dmul_rn(c, p);   // the rounded product, so that N = 1 gives exactly 0
+                    }
+                    partial0[(long long)slot * N + i] = pre * f0[r];
+                } else {
+                    partial0[(long long)slot * N + i] = pre * f0[r];
+                    partial1[(long long)slot * N + i] = pre * f1[r];
                 }
             }
         }
     });
-
-#pragma unroll
-    for (int r = 0; r < kPairR; ++r) {
-        const long long i = ibase + (long long)r * kPairThreads;
-        if (i < N) {
-            if (MODEL == 1) {
-                if (i >= jbeg && i < jend) {   // remove the rounding-level j = i term again
-                    double ny, y2;
-                    ring_pair_parts(a[r], b[r], make_double2(a[r], b[r]), onepe, ny, y2);
-                    f0[r] -= __dmul_rn(ny, y2);   // the rounded product, so that N = 1 gives exactly 0
-                }
-                partial0[(long long)s * N + i] = pre * f0[r];
-            } else {
-                partial0[(long long)s * N + i] = pre * f0[r];
-                partial1[(long long)s * N + i] = pre * f1[r];
-            }
-        }
-    }
 }
 
 // ---- potential-energy kernels (rows a-E2, a-E3) ---------------------------------------------------------
-// Full N x N sweep with the same tiling; the j = i term is masked out; the CTA writes
-// vpart[blockIdx.y * gridDim.x + blockIdx.x] = pre_half * sum_{i in tile} sum_{j in chunk, j != i} t_ij
+// Full N x N sweep with the same partition; the j = i term is masked out; CTA k writes
+// vpart[k] = pre_half * sum over its ranges of sum_{i in tile} sum_{j in range, j != i} t_ij
 // where pre_half already contains the 1/2 for double counting.
 //   Ring  t_ij = d_ij^(-1/2),  V = -(1/(sqrt2 N)) sum_{i<j} t_ij             eq.(1)
 //   2D    t_ij = log(r_ij^2 + eps), V = (1/N) sum_{i<j} t_ij                 eq.(3)
 // 2D uses sum log d = log prod d: one DMUL per pair into a running product whose exponent is
 // moved into an integer counter every 8 pairs (needs 2^-127 <= d <= 2^127), one log() per tile.
-template <int MODEL>
-__global__ void __launch_bounds__(kPairThreads, kPairCtasPerSm)
-pair_energy_kernel(const double2* __restrict__ js, long long N, double eps, double pre_half,
+template <int MODEL, typename CFG>
+__global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
+pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, double pre_half,
                    double* __restrict__ vpart) {
-    __shared__ PairSmem sm;
-    __shared__ double scratch[kPairThreads / 32];
-    const long long ibase = (long long)blockIdx.x * kPairITile + threadIdx.x;
-    const int S = gridDim.y, s = blockIdx.y;
-    long long jbeg, jend;
-    jchunk_bounds(N, S, s, jbeg, jend);
-
-    double a[kPairR], b[kPairR], acc[kPairR], prod[kPairR];
-    long long irow[kPairR];
-#pragma unroll
-    for (int r = 0; r < kPairR; ++r) {
-        const long long i = ibase + (long long)r * kPairThreads;
-        irow[r] = i;
-        const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
-        a[r] = q.x;
-        b[r] = q.y;
-        acc[r] = 0.0;
-        prod[r] = 1.0;
-    }
+    constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
+    __shared__ PairSmem<TJ> sm;
+    __shared__ double scratch[THREADS / 32];
+    JTilePipe<TJ> pipe(sm);
+    pipe.init();
+    const long long N = P.N;
     const double onepe = 1.0 + eps;
     constexpr double kLn2 = 0x1.62e42fefa39efp-1;
+    double vsum = 0.0;
 
-    for_each_jtile(sm, js, jbeg, jend, [&](const double2* tile, int cnt, long long j0) {
-        if (MODEL == 1) {
-#pragma unroll 4
-            for (int jj = 0; jj < cnt; ++jj) {
-                const double2 q = tile[jj];
+    for_each_segment(P, blockIdx.x, [&](long long tile, long long jbeg, long long jend, int) {
+        const long long ibase = tile * CFG::ITILE + threadIdx.x;
+        double a[R], b[R], acc[R], prod[R];
+        long long irow[R];
 #pragma unroll
-                for (int r = 0; r < kPairR; ++r) {
-                    const double d = fma(-b[r], q.y, fma(-a[r], q.x, onepe));
-                    const double y = rsqrt_refined(d);
-                    acc[r] += (irow[r] == j0 + jj) ? 0.0 : y;
-                }
-            }
-        } else {
-            int esum[kPairR];
-#pragma unroll
-            for (int r = 0; r < kPairR; ++r) esum[r] = 0;
-            for (int jb = 0; jb < cnt; jb += 8) {
-                const int m = (cnt - jb < 8) ? (cnt - jb) : 8;
-                if (m == 8) {
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) {
-                        const double2 q = tile[jb + u];
-#pragma unroll
-                        for (int r = 0; r < kPairR; ++r) {
-                            const double dx = a[r] - q.x, dy = b[r] - q.y;
-                            double d = fma(dy, dy, fma(dx, dx, eps));
-                            d = (irow[r] == j0 + jb + u) ? 1.0 : d;
-                            prod[r] *= d;
-                        }
-                    }
-                } else {
-                    for (int u = 0; u < m; ++u) {
-                        const double2 q = tile[jb + u];
-#pragma unroll
-                        for (int r = 0; r < kPairR; ++r) {
-                            const double dx = a[r] - q.x, dy = b[r] - q.y;
-                            double d = fma(dy, dy, fma(dx, dx, eps));
-                            d = (irow[r] == j0 + jb + u) ? 1.0 : d;
-                            prod[r] *= d;
-                        }
-                    }
-                }
-#pragma unroll
-                for (int r = 0; r < kPairR; ++r) {   // move the exponent into the integer counter
-                    const int hi = __double2hiint(prod[r]);
-                    esum[r] += ((hi >> 20) & 0x7ff) - 1023;
-                    prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
-                }
-            }
-#pragma unroll
-            for (int r = 0; r < kPairR; ++r) {
-                acc[r] += fma((double)esum[r], kLn2, log(prod[r]));
-                prod[r] = 1.0;
-            }
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            irow[r] = i;
+            const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
+            a[r] = q.x;
+            b[r] = q.y;
+            acc[r] = 0.0;
+            prod[r] = 1.0;
         }
+        pipe.run(js, jbeg, jend, [&](const double2* tl, int cnt, long long j0) {
+            if (MODEL == 1) {
+#pragma unroll 4
+                for (int jj = 0; jj < cnt; ++jj) {
+                    const double2 q = tl[jj];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const double d = fma(-b[r], q.y, fma(-a[r], q.x, onepe));
+                        const double y = rsqrt_refined(d);
+                        acc[r] += (irow[r] == j0 + jj) ? 0.0 : y;
+                    }
+                }
+            } else {
+                int esum[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) esum[r] = 0;
+                for (int jb = 0; jb < cnt; jb += 8) {
+                    const int m = (cnt - jb < 8) ? (cnt - jb) : 8;
+                    if (m == 8) {
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const double2 q = tl[jb + u];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double dx = a[r] - q.x, dy = b[r] - q.y;
+                                double d = fma(dy, dy, fma(dx, dx, eps));
+                                d = (irow[r] == j0 + jb + u) ? 1.0 : d;
+                                prod[r] *= d;
+                            }
+                        }
+                    } else {
+                        for (int u = 0; u < m; ++u) {
+                            const double2 q = tl[jb + u];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double dx = a[r] - q.x, dy = b[r] - q.y;
+                                double d = fma(dy, dy, fma(dx, dx, eps));
+                                d = (irow[r] == j0 + jb + u) ? 1.0 : d;
+                                prod[r] *= d;
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {   // move the exponent into the integer counter
+                        const int hi = __double2hiint(prod[r]);
+                        esum[r] += ((hi >> 20) & 0x7ff) - 1023;
+                        prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
+                    }
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    acc[r] += fma((double)esum[r], kLn2, log(prod[r]));
+                    prod[r] = 1.0;
+                }
+            }
+        });
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (irow[r] < N) vsum += acc[r];
     });
 
-    double v[1] = {0.0};
-#pragma unroll
-    for (int r = 0; r < kPairR; ++r)
-        if (irow[r] < N) v[0] += acc[r];
-    block_sum<kPairThreads, 1>(v, scratch);
-    if (threadIdx.x == 0) vpart[(long long)blockIdx.y * gridDim.x + blockIdx.x] = pre_half * v[0];
+    double v[1] = {vsum};
+    block_sum<THREADS, 1>(v, scratch);
+    if (threadIdx.x == 0) vpart[blockIdx.x] = pre_half * v[0];
 }
 
 // ---- update kernels (row a-U1) --------------------------------------------------------------------------
@@ -292,15 +375,24 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
     }
 }
 
-// f = sum_s partial[s][i] (index order); p += kickA f [; p += kickB f]; if DRIFT: q += drift p and
+// Number of partial rows of particle i's tile (the CTAs first..last of the partition touch it).
+__device__ __forceinline__ int tile_slots(const PairPart& P, long long i) {
+    long long first, last;
+    part_tile_ctas(P, i / P.itile, first, last);
+    return (int)(last - first + 1);
+}
+
+// f = sum_s partial[s][i] (slot order); p += kickA f [; p += kickB f]; if DRIFT: q += drift p and
 // the packed j-stream is refreshed (listing steps 2-3, 5-6, 8-9, 11; "update kernel").
 template <int MODEL, bool KICK2, bool DRIFT>
 __global__ void __launch_bounds__(kUpdThreads)
 pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __restrict__ p0, double* __restrict__ p1,
-                   long long N, const double* __restrict__ partial0, const double* __restrict__ partial1, int S,
+                   PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
                    double kickA, double kickB, double drift, double2* __restrict__ js) {
+    const long long N = P.N;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
+    const int S = tile_slots(P, i);
     double f = partial0[i];
     for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
     double p = fma(kickA, f, p0[i]);
@@ -331,10 +423,12 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
 
 // lrmd_forces for the pair models: f = sum_s partial[s][i]
 __global__ void __launch_bounds__(kUpdThreads)
-pair_force_out_kernel(long long N, const double* __restrict__ partial0, const double* __restrict__ partial1, int S,
+pair_force_out_kernel(PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
                       double* __restrict__ f0, double* __restrict__ f1) {
+    const long long N = P.N;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
+    const int S = tile_slots(P, i);
     double f = partial0[i];
     for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
     f0[i] = f;

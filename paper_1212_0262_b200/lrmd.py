@@ -17,13 +17,15 @@ import os
 
 HMF, RING, GRAV2D = 0, 1, 2
 OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
-OPT_PAIR_PRECISION, OPT_JSPLIT, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
+OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
+OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS = 5, 6, 7
 
 #: every symbol include/lrmd.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
+    "lrmd_pair_partition",
 )
 
 _lib = None
@@ -73,6 +75,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_strerror.restype = C.c_char_p
     lib.lrmd_coefficients.argtypes = [C.POINTER(_dbl)]
     lib.lrmd_host_sincos.argtypes = [_vp, _i64, _vp, _vp]
+    lib.lrmd_pair_partition.argtypes = [_vp, _i64, _vp, _i64, C.POINTER(_i64)]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int
@@ -179,6 +182,18 @@ def lrmd_host_sincos(x):
     if rc != OK:
         raise LrmdError(rc, "lrmd_host_sincos")
     return s, c
+
+
+def lrmd_pair_partition(ctx, cta: int, max_seg: int = 64):
+    """Diagnostic: (rc, segments) of CTA ``cta`` of the pair kernels; segments is an (n, 4) int64 numpy
+    array of rows {tile, jbeg, jend, slot}."""
+    import numpy as np
+    buf = np.zeros((max(max_seg, 1), 4), dtype=np.int64)
+    n = _i64(0)
+    rc = load().lrmd_pair_partition(ctx, int(cta), buf.ctypes.data, int(max_seg), C.byref(n))
+    if rc == OK and n.value > max_seg:
+        return lrmd_pair_partition(ctx, cta, int(n.value))
+    return rc, buf[: n.value].copy()
 
 
 # ---- convenience object ---------------------------------------------------------------------------------

@@ -69,18 +69,24 @@ def test_calls_before_state_and_workspace_are_estate(lrmd):
 
 def test_options(lrmd):
     rc, h = lrmd.lrmd_create(RING, 16384, 0.01)
-    rc, S = lrmd.lrmd_get_option(h, lrmd.OPT_JSPLIT)
-    assert rc == lrmd.OK and 1 <= S <= 64
-    assert lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, 3) == lrmd.OK
-    assert lrmd.lrmd_get_option(h, lrmd.OPT_JSPLIT) == (lrmd.OK, 3)
-    assert lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, -2) == lrmd.EINVAL
+    rc, G = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)
+    assert rc == lrmd.OK and G % 148 == 0 and G >= 148   # whole waves of the 148 SMs
+    rc, slots = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)
+    assert rc == lrmd.OK and 1 <= slots <= 64
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, 3) == lrmd.OK
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS) == (lrmd.OK, 3)
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS) == (lrmd.OK, 2)   # ranges longer than N: a tile meets <= 2 CTAs
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, -2) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, 99, 0) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_HMF_GRID, 8) == lrmd.EINVAL   # not an HMF context
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_HMF_VARIANT, 1) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_VARIANT, 9999) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 2) == lrmd.EINVAL
     rc, b3 = lrmd.lrmd_workspace_bytes(h)
-    lrmd.lrmd_set_option(h, lrmd.OPT_JSPLIT, 6)
+    lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, 32 * 6)
     rc, b6 = lrmd.lrmd_workspace_bytes(h)
-    assert b6 > b3                                     # partial-force rows grow with the j-split
+    assert b6 > b3                                     # partial-force rows grow with the number of CTAs per tile
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)[1] in (6, 7)   # 6 equal ranges per tile, boundaries not tile-aligned
     lrmd.lrmd_destroy(h)
     rc, h = lrmd.lrmd_create(HMF, 50_000_000, 0.0)
     rc, g = lrmd.lrmd_get_option(h, lrmd.OPT_HMF_GRID)
@@ -88,6 +94,59 @@ def test_options(lrmd):
     lrmd.lrmd_destroy(h)
     rc, h = lrmd.lrmd_create(HMF, 5, 0.0)
     assert lrmd.lrmd_get_option(h, lrmd.OPT_HMF_GRID)[1] >= 1
+    lrmd.lrmd_destroy(h)
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N,G", [(1, 0), (2, 0), (700, 0), (3000, 0), (16384, 0), (65536, 0), (3000, 1), (3000, 7),
+                                 (3000, 18000), (5000, 999), (1_048_576, 0), (200_003, 4321)])
+def test_pair_partition_covers_every_pair_once(lrmd, model, N, G):
+    """Host logic of the pair kernels' work partition (every ordered pair is computed):
+    the CTAs' segments tile each i-tile's j-range [0, N) exactly once and in order, each CTA's share of
+    pairs differs by at most one j-position, and slot numbers are 0..k-1 per tile with k <= PAIR_SLOTS."""
+    rc, h = lrmd.lrmd_create(model, N, 1e-3)
+    assert rc == lrmd.OK
+    if G:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, G) == lrmd.OK
+    ctas = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)[1]
+    slots = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)[1]
+    assert ctas >= 1 and (G == 0 or ctas == min(G, ctas))
+    if ctas > 3000:     # sample the CTAs of a large grid: the first, the last and a stride in between
+        pick = sorted(set([0, 1, ctas - 2, ctas - 1] + list(range(0, ctas, max(1, ctas // 997)))))
+    else:
+        pick = list(range(ctas))
+    lengths, per_tile = [], {}
+    prev_end = None
+    for k in pick:
+        rc, seg = lrmd.lrmd_pair_partition(h, k)
+        assert rc == lrmd.OK and len(seg) >= 1
+        lengths.append(int((seg[:, 2] - seg[:, 1]).sum()))
+        for tile, jb, je, slot in seg:
+            assert 0 <= jb < je <= N and 0 <= slot < slots
+            per_tile.setdefault(int(tile), []).append((int(jb), int(je), int(slot)))
+        # consecutive segments of one CTA continue into the next tile at j = 0
+        for a, b in zip(seg[:-1], seg[1:]):
+            assert a[2] == N and b[1] == 0 and b[0] == a[0] + 1
+        if prev_end is not None and k == prev_end[0] + 1:      # consecutive CTAs continue where the last ended
+            t, je = prev_end[1], prev_end[2]
+            assert (seg[0][0], seg[0][1]) == ((t, je) if je < N else (t + 1, 0))
+        prev_end = (k, int(seg[-1][0]), int(seg[-1][2]))
+    assert max(lengths) - min(lengths) <= 1
+    if len(pick) == ctas:
+        itile = None
+        ntiles = len(per_tile)
+        assert sorted(per_tile) == list(range(ntiles))
+        for t, segs in per_tile.items():
+            assert segs[0][0] == 0 and segs[-1][1] == N
+            assert [s[2] for s in segs] == list(range(len(segs)))
+            for a, b in zip(segs[:-1], segs[1:]):
+                assert a[1] == b[0]
+        assert sum(lengths) == ntiles * N
+    assert lrmd.lrmd_pair_partition(h, ctas)[0] == lrmd.EINVAL
+    assert lrmd.lrmd_pair_partition(h, -1)[0] == lrmd.EINVAL
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(HMF, 100, 0.0)
+    assert lrmd.lrmd_pair_partition(h, 0)[0] == lrmd.EINVAL
     lrmd.lrmd_destroy(h)
 
 

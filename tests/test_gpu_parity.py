@@ -86,15 +86,15 @@ def test_forces_match_oracle_small_and_ragged(lrmd, ref, torch, model, N):
 
 
 @pytest.mark.parametrize("model", [RING, GRAV2D])
-@pytest.mark.parametrize("S", [1, 2, 3, 7, 16])
-def test_forces_any_jsplit(lrmd, ref, torch, model, S):
-    """The (i-tile x j-chunk) grid with partial-force rows summed in index order (row a-U1)."""
+@pytest.mark.parametrize("S", [1, 2, 3, 7, 16, 148, 1000, 12500])
+def test_forces_any_partition(lrmd, ref, torch, model, S):
+    """Any number of CTAs over the flattened (i-tile, j) space; partial-force rows summed in slot order (row a-U1)."""
     eps = _eps(model)
     N = 2500
     st = _state(model, N, 77)
     q0, q1 = _q(model, st)
     f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
-    got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_JSPLIT: S})
+    got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_PAIR_CTAS: S})
     _check_forces(model, got, (f0, f1), (A0, A1))
 
 
@@ -106,6 +106,66 @@ def test_hmf_forces_any_grid(lrmd, ref, torch, grid):
     got = _gpu_forces(lrmd, HMF, 0.0, st, options={lrmd.OPT_HMF_GRID: grid})
     # at this N use the pair-sum-free bound: A_i is within a factor ~2 of S_i for a waterbag
     assert np.all(np.abs(got[0] - f0) <= FTOL * 0.5 * S0)
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("N", [1, 2, 7, 2047, 2048, 2049, 300_001])
+def test_hmf_tma_variants_match_oracle(lrmd, ref, torch, variant, N):
+    """TMA-staged fused substage (persistent CTAs, smem ring, bulk loads and stores): forces and a
+    3-step trajectory against the oracle; odd N exercises the scalar tail, N < chunk the short copies."""
+    st = _state(HMF, N, 700 + N % 97)
+    f0, _, S0, _ = ref.forces_abs(HMF, 0.0, st[0], None, form=0)
+    ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: variant, lrmd.OPT_GRAPH: 0})
+    ctx.set_state(*st)
+    got = ctx.forces().cpu().numpy()
+    assert np.all(np.abs(got - f0) <= FTOL * S0 + 4e-16)
+    ctx.step(3, 0.05)
+    e = ctx.energy().cpu().numpy()
+    out = ctx.state_numpy()
+    ctx.close()
+    th, p = st[0].copy(), st[1].copy()
+    ref.step(HMF, 0.0, th, None, p, None, 3, 0.05, form=0)
+    assert np.max(np.abs(out[0] - th)) <= XTOL and np.max(np.abs(out[1] - p)) <= XTOL
+    er, ea = ref.energy(HMF, 0.0, th, None, p, None)
+    assert abs(e[0] - er[0]) <= 1e-12 * ea[0] + 1e-300
+    assert abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N) + 1e-300
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_hmf_tma_variant_graph_and_grid(lrmd, torch, variant):
+    """Graph replay and a non-default grid give the same bits as plain launches of the same variant and grid."""
+    N = 40_001
+    st = _state(HMF, N, 3)
+    outs = []
+    for graph in (0, 1):
+        ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: variant, lrmd.OPT_GRAPH: graph, lrmd.OPT_HMF_GRID: 5})
+        ctx.set_state(*st)
+        ctx.step(20, 0.05)
+        outs.append(ctx.state_numpy())
+        ctx.close()
+    for x, y in zip(*outs):
+        assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_pair_variants_match_oracle(lrmd, ref, torch, model, variant):
+    """Every compiled launch shape of the pair kernels: forces and potential energy against the oracle."""
+    eps = _eps(model)
+    N = 3333
+    st = _state(model, N, 55)
+    q0, q1 = _q(model, st)
+    p0, p1 = _p(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_VARIANT: variant})
+    ctx.set_state(*st)
+    f = ctx.forces()
+    got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    e = ctx.energy().cpu().numpy()
+    ctx.close()
+    _check_forces(model, got, (f0, f1), (A0, A1))
+    e_ref, e_abs = ref.energy(model, eps, q0, q1, p0, p1)
+    assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
 
 
 @pytest.mark.parametrize("model,eps", [(RING, 1e-3), (RING, 1.0), (RING, 1e4), (GRAV2D, 1e-6), (GRAV2D, 10.0)])
@@ -279,15 +339,15 @@ def test_energy_matches_oracle(lrmd, ref, torch, model, N):
     assert abs(e[3] - e_ref[3]) <= 1e-12 * max(1.0, np.sum(np.abs(p1)) if p1 is not None else 1.0)
 
 
-@pytest.mark.parametrize("S", [1, 5])
-def test_energy_any_jsplit(lrmd, ref, torch, S):
+@pytest.mark.parametrize("S", [1, 5, 333])
+def test_energy_any_partition(lrmd, ref, torch, S):
     for model in (RING, GRAV2D):
         eps = _eps(model)
         st = _state(model, 3000, 41)
         q0, q1 = _q(model, st)
         p0, p1 = _p(model, st)
         e_ref, e_abs = ref.energy(model, eps, q0, q1, p0, p1)
-        ctx = lrmd.Context(model, 3000, eps, options={lrmd.OPT_JSPLIT: S})
+        ctx = lrmd.Context(model, 3000, eps, options={lrmd.OPT_PAIR_CTAS: S})
         ctx.set_state(*st)
         e = ctx.energy().cpu().numpy()
         ctx.close()
