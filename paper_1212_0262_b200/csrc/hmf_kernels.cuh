@@ -50,12 +50,57 @@ __device__ __forceinline__ void hmf_magnetisation(const double2* __restrict__ pa
     My = v[1] * inv_n;
 }
 
+// sin / cos of four angles.  One range check for the group keeps the common path free of branches
+// (the kernel is limited by instruction issue as much as by HBM); a group with an angle beyond
+// 2^30 takes the checked per-particle form, which gives every particle the same bits either way.
+__device__ __forceinline__ void sincos4(const double (&x)[4], double (&s)[4], double (&c)[4]) {
+    if (sincos_is_small(x[0]) && sincos_is_small(x[1]) && sincos_is_small(x[2]) && sincos_is_small(x[3])) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) sincos_fast(x[k], s[k], c[k]);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double2 r = sincos_any_call(x[k]);
+            s[k] = r.x;
+            c[k] = r.y;
+        }
+    }
+}
+
+// One substage for four particles: kick with the force at the current angles, drift, and the
+// cos / sin terms of the new angles added to the thread's partial sums (particles 0,1 count if
+// v01, particles 2,3 if v23: invalid slots carry zeros and are computed but not summed).
+template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
+__device__ __forceinline__ void hmf_group4(double (&th)[4], double (&p)[4], bool v01, bool v23, double Mx, double My,
+                                           double kickA, double kickB, double drift, double& accC, double& accS) {
+    double s[4], c[4];
+    if (KICK) {
+        sincos4(th, s, c);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double f = fma(c[k], My, -(s[k] * Mx));
+            p[k] = fma(kickA, f, p[k]);
+            if (KICK2) p[k] = fma(kickB, f, p[k]);
+        }
+    }
+    if (DRIFT) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) th[k] = fma(drift, p[k], th[k]);
+    }
+    if (REDUCE) {
+        sincos4(th, s, c);
+        if (v01) { accC += c[0]; accS += s[0]; accC += c[1]; accS += s[1]; }
+        if (v23) { accC += c[2]; accS += s[2]; accC += c[3]; accS += s[3]; }
+    }
+}
+
+// One particle (ragged tails).
 template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
 __device__ __forceinline__ void hmf_particle(double& th, double& p, double Mx, double My, double kickA, double kickB,
                                              double drift, double& accC, double& accS) {
     if (KICK) {
         double s, c;
-        sincos_pi4(th, s, c);
+        sincos_any(th, s, c);
         const double f = fma(c, My, -(s * Mx));
         p = fma(kickA, f, p);
         if (KICK2) p = fma(kickB, f, p);
@@ -63,7 +108,7 @@ __device__ __forceinline__ void hmf_particle(double& th, double& p, double Mx, d
     if (DRIFT) th = fma(drift, p, th);
     if (REDUCE) {
         double s, c;
-        sincos_pi4(th, s, c);
+        sincos_any(th, s, c);
         accC += c;
         accS += s;
     }
@@ -98,12 +143,12 @@ hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long lon
             tn = ld256(theta + 4 * vn);
             if (KICK || DRIFT) pn = ld256(p + 4 * vn);
         }
-        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.a, p4.a, Mx, My, kickA, kickB, drift, accC, accS);
-        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.b, p4.b, Mx, My, kickA, kickB, drift, accC, accS);
-        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.c, p4.c, Mx, My, kickA, kickB, drift, accC, accS);
-        hmf_particle<KICK, KICK2, DRIFT, REDUCE>(t4.d, p4.d, Mx, My, kickA, kickB, drift, accC, accS);
-        if (DRIFT) st256(theta + 4 * v, t4);
-        if (KICK) st256(p + 4 * v, p4);
+        {
+            double tt[4] = {t4.a, t4.b, t4.c, t4.d}, pp[4] = {p4.a, p4.b, p4.c, p4.d};
+            hmf_group4<KICK, KICK2, DRIFT, REDUCE>(tt, pp, true, true, Mx, My, kickA, kickB, drift, accC, accS);
+            if (DRIFT) st256(theta + 4 * v, dbl4{tt[0], tt[1], tt[2], tt[3]});
+            if (KICK) st256(p + 4 * v, dbl4{pp[0], pp[1], pp[2], pp[3]});
+        }
         t4 = tn;
         p4 = pn;
         v = vn;
@@ -226,13 +271,13 @@ hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long
             double2 ta = make_double2(0.0, 0.0), tb = ta, pa = ta, pb = ta;
             if (h0) { ta = t2[u0]; if (LOADP) pa = p2[u0]; }
             if (h1) { tb = t2[u1]; if (LOADP) pb = p2[u1]; }
-            if (h0) {
-                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(ta.x, pa.x, Mx, My, kickA, kickB, drift, accC, accS);
-                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(ta.y, pa.y, Mx, My, kickA, kickB, drift, accC, accS);
-            }
-            if (h1) {
-                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(tb.x, pb.x, Mx, My, kickA, kickB, drift, accC, accS);
-                hmf_particle<KICK, KICK2, DRIFT, REDUCE>(tb.y, pb.y, Mx, My, kickA, kickB, drift, accC, accS);
+            {
+                double tt[4] = {ta.x, ta.y, tb.x, tb.y}, pp[4] = {pa.x, pa.y, pb.x, pb.y};
+                hmf_group4<KICK, KICK2, DRIFT, REDUCE>(tt, pp, h0, h1, Mx, My, kickA, kickB, drift, accC, accS);
+                ta = make_double2(tt[0], tt[1]);
+                tb = make_double2(tt[2], tt[3]);
+                pa = make_double2(pp[0], pp[1]);
+                pb = make_double2(pp[2], pp[3]);
             }
             if (STORE) {
                 if (h0) { if (STORE_TH) t2[u0] = ta; if (STORE_P) p2[u0] = pa; }
@@ -268,7 +313,7 @@ hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long 
     const long long stride = (long long)gridDim.x * kHmfThreads;
     for (long long i = (long long)blockIdx.x * kHmfThreads + threadIdx.x; i < N; i += stride) {
         double s, c;
-        sincos_pi4(theta[i], s, c);
+        sincos_any(theta[i], s, c);
         f[i] = fma(c, My, -(s * Mx));
     }
 }

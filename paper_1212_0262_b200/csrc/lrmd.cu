@@ -82,7 +82,7 @@ namespace {
 // HMF: variant 0 is the register-prefetch kernel (best below ~1e6 particles, where the step is latency
 // bound), the others the TMA-staged kernel <consumer threads, stages, CTAs per SM>.
 struct HmfVariant { int consumers, stages, minb; };
-constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 3, 2}, {512, 4, 1}, {480, 3, 2}};
+constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}};
 constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
 constexpr int64_t kHmfTmaMinN = 1000000;
 
@@ -294,9 +294,8 @@ void hmf_launch(Launcher& L, bool timed, double kickA, double kickB, double drif
         LRMD_HMF_GO((hmf_substage_tma_kernel<KICK, KICK2, DRIFT, REDUCE, CONS, NS, MINB>), CONS + 32);       \
         break
     switch (c->hmf_variant) {
-        LRMD_HMF_TMA(1, 512, 3, 2);
-        LRMD_HMF_TMA(2, 512, 4, 1);
-        LRMD_HMF_TMA(3, 480, 3, 2);
+        LRMD_HMF_TMA(1, 512, 4, 1);
+        LRMD_HMF_TMA(2, 256, 6, 2);
         default:
             LRMD_HMF_GO((hmf_substage_kernel<KICK, KICK2, DRIFT, REDUCE>), kHmfThreads);
             break;
@@ -716,7 +715,10 @@ int lrmd_pair_partition(const lrmd_ctx* c, int64_t cta, int64_t* seg4_host, int6
     if (!c || !nseg_host || c->model == LRMD_HMF || cta < 0 || cta >= c->part.G || max_seg < 0) return LRMD_EINVAL;
     if (max_seg > 0 && !seg4_host) return LRMD_EINVAL;
     int64_t n = 0;
-    for_each_segment(c->part, (long long)cta, [&](long long tile, long long jbeg, long long jend, int slot) {
+    PairSegments segs(c->part, (long long)cta);
+    long long tile, jbeg, jend;
+    int slot;
+    while (segs.next(c->part, tile, jbeg, jend, slot)) {
         if (n < max_seg) {
             seg4_host[4 * n + 0] = tile;
             seg4_host[4 * n + 1] = jbeg;
@@ -724,14 +726,14 @@ int lrmd_pair_partition(const lrmd_ctx* c, int64_t cta, int64_t* seg4_host, int6
             seg4_host[4 * n + 3] = slot;
         }
         ++n;
-    });
+    }
     *nseg_host = n;
     return LRMD_OK;
 }
 
 int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host) {
     if (!x_host || !s_host || !c_host || n < 0) return LRMD_EINVAL;
-    for (int64_t i = 0; i < n; ++i) sincos_pi4(x_host[i], s_host[i], c_host[i]);
+    for (int64_t i = 0; i < n; ++i) sincos_any(x_host[i], s_host[i], c_host[i]);
     return LRMD_OK;
 }
 

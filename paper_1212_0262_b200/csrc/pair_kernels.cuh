@@ -158,20 +158,23 @@ struct JTilePipe {
     }
 };
 
-// Calls seg(tile, jbeg, jend, slot) for every (i-tile, j-range) segment of CTA k's range.
-template <typename Seg>
-__host__ __device__ __forceinline__ void for_each_segment(const PairPart& P, long long k, Seg seg) {
-    long long pos = part_bound(P, k);
-    const long long end = part_bound(P, k + 1);
-    while (pos < end) {
-        const long long t = pos / P.N;
-        const long long jbeg = pos - t * P.N;
-        const long long jend = (end - pos < P.N - jbeg) ? jbeg + (end - pos) : P.N;
-        const int slot = (int)(k - part_owner(P, t * P.N));
-        seg(t, jbeg, jend, slot);
+// Iterates over the (i-tile, j-range) segments of CTA k's range: next() yields the pairs
+// (i in tile) x (jbeg <= j < jend) and the partial force row `slot` they are added into.
+struct PairSegments {
+    long long pos, end, k;
+    __host__ __device__ __forceinline__ PairSegments(const PairPart& P, long long cta)
+        : pos(part_bound(P, cta)), end(part_bound(P, cta + 1)), k(cta) {}
+    __host__ __device__ __forceinline__ bool next(const PairPart& P, long long& tile, long long& jbeg, long long& jend,
+                                                  int& slot) {
+        if (pos >= end) return false;
+        tile = pos / P.N;
+        jbeg = pos - tile * P.N;
+        jend = (end - pos < P.N - jbeg) ? jbeg + (end - pos) : P.N;
+        slot = (int)(k - part_owner(P, tile * P.N));
         pos += jend - jbeg;
+        return true;
     }
-}
+};
 
 // ---- force kernels (rows a-P1r, a-P1g) --------------------------------------------------------------
 
@@ -187,7 +190,10 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
     const long long N = P.N;
     const double onepe = 1.0 + eps;
 
-    for_each_segment(P, blockIdx.x, [&](long long tile, long long jbeg, long long jend, int slot) {
+    PairSegments segs(P, blockIdx.x);
+    long long tile, jbeg, jend;
+    int slot;
+    while (segs.next(P, tile, jbeg, jend, slot)) {
         const long long ibase = tile * CFG::ITILE + threadIdx.x;
         double a[R], b[R], f0[R], f1[R];
 #pragma unroll
@@ -251,7 +257,7 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
                 }
             }
         }
-    });
+    }
 }
 
 // ---- potential-energy kernels (rows a-E2, a-E3) ---------------------------------------------------------
@@ -276,7 +282,10 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
     constexpr double kLn2 = 0x1.62e42fefa39efp-1;
     double vsum = 0.0;
 
-    for_each_segment(P, blockIdx.x, [&](long long tile, long long jbeg, long long jend, int) {
+    PairSegments segs(P, blockIdx.x);
+    long long tile, jbeg, jend;
+    int slot;
+    while (segs.next(P, tile, jbeg, jend, slot)) {
         const long long ibase = tile * CFG::ITILE + threadIdx.x;
         double a[R], b[R], acc[R], prod[R];
         long long irow[R];
@@ -349,7 +358,7 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (irow[r] < N) vsum += acc[r];
-    });
+    }
 
     double v[1] = {vsum};
     block_sum<THREADS, 1>(v, scratch);
@@ -368,7 +377,7 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
     if (i >= N) return;
     if (MODEL == 1) {
         double s, c;
-        sincos_pi4(q0[i], s, c);
+        sincos_any(q0[i], s, c);
         js[i] = make_double2(c, s);
     } else {
         js[i] = make_double2(q0[i], q1[i]);
@@ -415,7 +424,7 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
             js[i] = make_double2(x, y);
         } else {
             double sn, cs;
-            sincos_pi4(x, sn, cs);
+            sincos_any(x, sn, cs);
             js[i] = make_double2(cs, sn);
         }
     }

@@ -108,7 +108,7 @@ def test_hmf_forces_any_grid(lrmd, ref, torch, grid):
     assert np.all(np.abs(got[0] - f0) <= FTOL * 0.5 * S0)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 2])
 @pytest.mark.parametrize("N", [1, 2, 7, 2047, 2048, 2049, 300_001])
 def test_hmf_tma_variants_match_oracle(lrmd, ref, torch, variant, N):
     """TMA-staged fused substage (persistent CTAs, smem ring, bulk loads and stores): forces and a
