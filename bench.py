@@ -123,14 +123,15 @@ def units_per_force(w):
     return "pair-interactions/s", "pair-interactions/s", float(w.N) * float(w.N)
 
 
-def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
+def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False):
     import torch
     from paper_1212_0262_b200 import lrmd
 
     dev = torch.device("cuda", torch.cuda.current_device())
     peaks = measured_peaks()
     st = w.state()
-    ctx = lrmd.Context(w.model, w.N, w.eps, device=dev)
+    ctx = lrmd.Context(w.model, w.N, w.eps, device=dev,
+                       options=({lrmd.OPT_PAIR_PRECISION: 1} if f32_pairs else None))
     ctx.set_state(*st)
     stream = torch.cuda.current_stream(dev)
     state_bytes = ctx.narrays * w.N * 8
@@ -198,7 +199,8 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
                if resident_by_design else "L2 flushed (256 MiB write) before every timed step"),
         "options": {"pair_ctas": ctx.get_option(lrmd.OPT_PAIR_CTAS), "pair_variant": ctx.get_option(lrmd.OPT_PAIR_VARIANT),
                     "pair_slots": ctx.get_option(lrmd.OPT_PAIR_SLOTS), "graph": ctx.get_option(lrmd.OPT_GRAPH),
-                    "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT)},
+                    "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT),
+                    "pair_precision": ctx.get_option(lrmd.OPT_PAIR_PRECISION)},
     }
 
     # ---- roofline of the dominant kernel: second pass with an event pair around each of its launches
@@ -217,6 +219,15 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
             roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
                     "algorithmic_bytes_per_launch": bytes_per_launch}
+        elif f32_pairs:
+            # fp32 pair arithmetic: one MUFU.RCP per pair on the special-function unit, 16 lanes per SM per clock
+            mufu = float(w.N) * float(w.N)
+            peak = SM_COUNT * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
+            achieved = mufu / avg_s / 1e12
+            roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T MUFU.RCP/s (= T pairs/s)",
+                    "frac": achieved / peak,
+                    "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: 6 FADD/FFMA per pair",
+                    "algorithmic_mufu_per_launch": mufu}
         else:
             flop = PAIR_FLOP[w.model] * w.N * w.N
             achieved = flop / avg_s / 1e12
@@ -227,7 +238,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True):
                     "algorithmic_flop_per_launch": flop,
                     "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
                     "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
-        roof.update({"kernel": "hmf_substage_kernel" if w.model == 0 else "pair_force_kernel",
+        roof.update({"kernel": "hmf_substage_kernel" if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else "pair_force_kernel"),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(w.key)})
@@ -338,6 +349,7 @@ def main():
     ap.add_argument("--only", action="store_true", help="primary workload only (no 'others', no cpu_baseline)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--f32-pairs", action="store_true", help="GRAV2D workloads: fp32 pair arithmetic (PAPER.md:110)")
     args = ap.parse_args()
 
     from paper_1212_0262_b200 import inputs
@@ -366,11 +378,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist_ctx = dist
 
-    res = run_workload(w, K, W, dist_ctx)
+    res = run_workload(w, K, W, dist_ctx, f32_pairs=bool(args.f32_pairs and w.model == 2))
     line = {
         "metric": res["metric"], "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "dtype": "f32" if (args.f32_pairs and w.model == 2) else "f64", "data": "synthetic",
         "config": {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt,
                    "step": "one 4th-order time step = 3 force evaluations + kick/drift updates (PAPER.md:54-63)",
                    "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
@@ -389,6 +401,12 @@ def main():
             others[key] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options",
                                               "clocks", "roofline", "e2e") if k in r}
             others[key]["steps"] = DEFAULT_STEPS[key]
+        # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
+        r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)
+        others["grav2d_1m_f32pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
+                                                           "options", "clocks", "roofline") if k in r}
+        others["grav2d_1m_f32pairs"]["steps"] = DEFAULT_STEPS["grav2d_1m"]
+        others["grav2d_1m_f32pairs"]["dtype"] = "f32 pair terms, f64 state and accumulation"
         line["others"] = others
         rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
         line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc}

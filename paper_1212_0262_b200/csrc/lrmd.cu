@@ -30,6 +30,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
     size_t hmf_partial = 0;   // 3 rotating buffers of kHmfMaxGrid double2 (HMF)
     size_t js = 0;            // packed j-stream double2[N] (pair models)
+    size_t js32 = 0;          // fp32 copy float2[N + pad] (GRAV2D, pair precision 1)
     size_t partial0 = 0;      // [slots][N] partial forces
     size_t partial1 = 0;      // [slots][N] (GRAV2D)
     size_t kpart = 0;         // 3 * kEnergyGrid
@@ -158,6 +159,7 @@ void resolve(lrmd_ctx* c) {
         c->slots = (int)smax;
         c->hmf_grid = 0;
         L.js = off; off = align_up(off + sizeof(double2) * (size_t)N);
+        if (c->opt_precision == 1) { L.js32 = off; off = align_up(off + sizeof(float2) * ((size_t)N + 2)); }
         L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots);
         if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots); }
         L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
@@ -259,6 +261,9 @@ inline double2* hmf_buf(lrmd_ctx* c, int k) {
     return reinterpret_cast<double2*>(c->ws + c->lay.hmf_partial) + (size_t)k * kHmfMaxGrid;
 }
 inline double2* js_ptr(lrmd_ctx* c) { return reinterpret_cast<double2*>(c->ws + c->lay.js); }
+inline float2* js32_ptr(lrmd_ctx* c) {
+    return c->opt_precision == 1 ? reinterpret_cast<float2*>(c->ws + c->lay.js32) : nullptr;
+}
 inline double* part0(lrmd_ctx* c) { return reinterpret_cast<double*>(c->ws + c->lay.partial0); }
 inline double* part1(lrmd_ctx* c) {
     return c->model == LRMD_GRAV2D ? reinterpret_cast<double*>(c->ws + c->lay.partial1) : nullptr;
@@ -381,8 +386,8 @@ int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
 void pair_pack(Launcher& L) {
     lrmd_ctx* c = L.c;
     const dim3 g((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), b(kUpdThreads);
-    if (c->model == LRMD_RING) L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, js_ptr(c));
-    else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, js_ptr(c));
+    if (c->model == LRMD_RING) L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, js_ptr(c), (float2*)nullptr);
+    else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, js_ptr(c), js32_ptr(c));
 }
 
 void pair_force(Launcher& L) {
@@ -393,6 +398,9 @@ void pair_force(Launcher& L) {
         if (c->model == LRMD_RING)
             L.go_timed(pair_force_kernel<1, CFG>, g, b, js_ptr(c), c->part, c->eps,
                        -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N), part0(c), part1(c));
+        else if (c->opt_precision == 1)
+            L.go_timed(grav_force_f32_kernel<CFG>, g, b, (const float2*)js32_ptr(c), c->part, (float)c->eps,
+                       -2.0 / (double)c->N, part0(c), part1(c));
         else
             L.go_timed(pair_force_kernel<2, CFG>, g, b, js_ptr(c), c->part, c->eps, -2.0 / (double)c->N, part0(c),
                        part1(c));
@@ -405,7 +413,7 @@ void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB
     double *q0 = c->a0, *q1 = nullptr, *p0 = c->a1, *p1 = nullptr;
     if (c->model == LRMD_GRAV2D) { q1 = c->a1; p0 = c->a2; p1 = c->a3; }
 #define LRMD_UPD(M, K2, DR) \
-    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, part0(c), part1(c), kickA, kickB, d, js_ptr(c))
+    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, part0(c), part1(c), kickA, kickB, d, js_ptr(c), js32_ptr(c))
     if (c->model == LRMD_RING) {
         if (!drift) LRMD_UPD(1, false, false);
         else if (kick2) LRMD_UPD(1, true, true);
@@ -609,9 +617,11 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
     if (!c) return LRMD_EINVAL;
     switch (key) {
         case LRMD_OPT_PAIR_PRECISION:
-            if (value == 0) break;
-            if (value == 1) return LRMD_EUNSUPPORTED;   // fp32-pair variant: SURVEY.md 8(f) N1, not built yet
-            return LRMD_EINVAL;
+            if (value != 0 && value != 1) return LRMD_EINVAL;
+            if (value == 1 && c->model != LRMD_GRAV2D) return LRMD_EUNSUPPORTED;   // fp32 pairs: GRAV2D only
+            if (value == 1 && !(c->eps >= 1e-30)) return LRMD_EUNSUPPORTED;        // eps must be a normal float
+            c->opt_precision = value;
+            break;
         case LRMD_OPT_PAIR_CTAS:
             if (value < 0 || value > (1 << 24)) return LRMD_EINVAL;
             if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
@@ -656,7 +666,7 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
 int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
     if (!c || !value) return LRMD_EINVAL;
     switch (key) {
-        case LRMD_OPT_PAIR_PRECISION: *value = 0; break;
+        case LRMD_OPT_PAIR_PRECISION: *value = c->opt_precision; break;
         case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : c->part.G; break;
         case LRMD_OPT_HMF_VARIANT: *value = c->hmf_variant; break;
         case LRMD_OPT_PAIR_VARIANT: *value = c->pair_variant; break;

@@ -108,20 +108,20 @@ __device__ __forceinline__ void ring_pair_parts(double ci, double si, double2 q,
 
 // ---- j-tile pipeline ----------------------------------------------------------------------------------
 
-template <int TJ>
+template <typename T, int TJ>
 struct PairSmem {
-    alignas(128) double2 tile[2][TJ];
+    alignas(128) T tile[2][TJ];
     alignas(8) uint64_t full[2];
 };
 
 // Two-stage ring of j-tiles filled by 1-D TMA bulk copies.  init() once per CTA; run() may be
 // called for several j-ranges in turn (every copy it issues is consumed before it returns, so the
 // barrier phases carry over).
-template <int TJ>
+template <typename T, int TJ>
 struct JTilePipe {
-    PairSmem<TJ>& sm;
+    PairSmem<T, TJ>& sm;
     uint32_t phases = 0u;   // bit s = parity the next wait on stage s expects
-    __device__ __forceinline__ explicit JTilePipe(PairSmem<TJ>& s) : sm(s) {}
+    __device__ __forceinline__ explicit JTilePipe(PairSmem<T, TJ>& s) : sm(s) {}
     __device__ __forceinline__ void init() {
         if (threadIdx.x == 0) {
             mbar_init(&sm.full[0], 1);
@@ -131,28 +131,37 @@ struct JTilePipe {
         __syncthreads();
     }
     // Calls body(tile_ptr, count, j0) for consecutive tiles of [jbeg, jend) of the packed j-stream.
+    // Bulk copies move multiples of 16 bytes from 16-byte aligned addresses: for 8-byte elements
+    // (the fp32 stream) the copies start at the even index at or below jbeg and end at the even
+    // index at or above jend (the array is padded to an even length), and body() is handed the
+    // valid part only.
     template <typename Body>
-    __device__ __forceinline__ void run(const double2* __restrict__ js, long long jbeg, long long jend, Body body) {
-        const int ntiles = (int)((jend - jbeg + TJ - 1) / TJ);
+    __device__ __forceinline__ void run(const T* __restrict__ js, long long jbeg, long long jend, Body body) {
+        constexpr long long A = 16 / sizeof(T);              // elements per 16 bytes: 1 (double2) or 2 (float2)
+        static_assert(A >= 1 && TJ % A == 0, "tile length must keep the copies aligned");
+        const long long ja = jbeg & ~(A - 1);
+        const long long je = (jend + A - 1) & ~(A - 1);
+        const int ntiles = (int)((je - ja + TJ - 1) / TJ);
         if (threadIdx.x == 0 && ntiles > 0) {
-            const long long c0 = (jend - jbeg < TJ) ? (jend - jbeg) : TJ;
-            mbar_expect_tx(&sm.full[0], (uint32_t)(c0 * sizeof(double2)));
-            bulk_g2s(sm.tile[0], js + jbeg, (uint32_t)(c0 * sizeof(double2)), &sm.full[0]);
+            const long long c0 = (je - ja < TJ) ? (je - ja) : TJ;
+            mbar_expect_tx(&sm.full[0], (uint32_t)(c0 * sizeof(T)));
+            bulk_g2s(sm.tile[0], js + ja, (uint32_t)(c0 * sizeof(T)), &sm.full[0]);
         }
         for (int t = 0; t < ntiles; ++t) {
             const int s = t & 1;
-            const long long j0 = jbeg + (long long)t * TJ;
+            const long long j0 = ja + (long long)t * TJ;
             if (threadIdx.x == 0 && t + 1 < ntiles) {
                 // stage s^1 was consumed in iteration t-1; every thread passed the barrier that ended it
                 const long long j1 = j0 + TJ;
-                const long long c1 = (jend - j1 < TJ) ? (jend - j1) : TJ;
-                mbar_expect_tx(&sm.full[s ^ 1], (uint32_t)(c1 * sizeof(double2)));
-                bulk_g2s(sm.tile[s ^ 1], js + j1, (uint32_t)(c1 * sizeof(double2)), &sm.full[s ^ 1]);
+                const long long c1 = (je - j1 < TJ) ? (je - j1) : TJ;
+                mbar_expect_tx(&sm.full[s ^ 1], (uint32_t)(c1 * sizeof(T)));
+                bulk_g2s(sm.tile[s ^ 1], js + j1, (uint32_t)(c1 * sizeof(T)), &sm.full[s ^ 1]);
             }
             mbar_wait(&sm.full[s], (phases >> s) & 1u);
             phases ^= 1u << s;
+            const int skip = (A > 1 && t == 0) ? (int)(jbeg - ja) : 0;
             const int cnt = (int)((jend - j0 < TJ) ? (jend - j0) : TJ);
-            body(sm.tile[s], cnt, j0);
+            body(sm.tile[s] + skip, cnt - skip, j0 + skip);
             __syncthreads();
         }
     }
@@ -184,8 +193,8 @@ __global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
 pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double pre,
                   double* __restrict__ partial0, double* __restrict__ partial1) {
     constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
-    __shared__ PairSmem<TJ> sm;
-    JTilePipe<TJ> pipe(sm);
+    __shared__ PairSmem<double2, TJ> sm;
+    JTilePipe<double2, TJ> pipe(sm);
     pipe.init();
     const long long N = P.N;
     const double onepe = 1.0 + eps;
@@ -260,6 +269,89 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
     }
 }
 
+// ---- 2D force, fp32 pair arithmetic ----------------------------------
+// The paper's mixed-precision variant: "the positions are copied to single precision variables in
+// shared memory, the force is computed in single precision and then summed to a double precision
+// variable".  Here: a second packed stream float2 xy32[] (positions rounded to fp32 by the update
+// kernel), pair terms in fp32 (4 FADD/FFMA for dx, dy, r^2 + eps; MUFU.RCP; 2 FFMA), summed in fp32
+// over at most kF32Chunk consecutive j and then added to the fp64 accumulators (reading G16: a
+// pure fp32 accumulator over 1e6 terms would miss the 1e-5 tolerance).  Bound by the special-
+// function unit: one MUFU.RCP per pair at 16 lanes per SM per clock.
+constexpr int kF32Chunk = 32;
+
+__device__ __forceinline__ float rcp_f32(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <typename CFG>
+__global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
+grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, double pre,
+                      double* __restrict__ partial0, double* __restrict__ partial1) {
+    constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
+    __shared__ PairSmem<float2, TJ> sm;
+    JTilePipe<float2, TJ> pipe(sm);
+    pipe.init();
+    const long long N = P.N;
+
+    PairSegments segs(P, blockIdx.x);
+    long long tile, jbeg, jend;
+    int slot;
+    while (segs.next(P, tile, jbeg, jend, slot)) {
+        const long long ibase = tile * CFG::ITILE + threadIdx.x;
+        float a[R], b[R];
+        double f0[R], f1[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            const float2 q = (i < N) ? js32[i] : make_float2(0.f, 0.f);
+            a[r] = q.x;
+            b[r] = q.y;
+            f0[r] = 0.0;
+            f1[r] = 0.0;
+        }
+        pipe.run(js32, jbeg, jend, [&](const float2* tl, int cnt, long long) {
+            for (int c0 = 0; c0 < cnt; c0 += kF32Chunk) {
+                const int m = (cnt - c0 < kF32Chunk) ? (cnt - c0) : kF32Chunk;
+                float sx[R], sy[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) sx[r] = sy[r] = 0.f;
+                auto pair = [&](const float2 q) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const float dx = a[r] - q.x;
+                        const float dy = b[r] - q.y;
+                        const float r2 = fmaf(dy, dy, fmaf(dx, dx, eps));
+                        const float w = rcp_f32(r2);
+                        sx[r] = fmaf(dx, w, sx[r]);
+                        sy[r] = fmaf(dy, w, sy[r]);
+                    }
+                };
+                if (m == kF32Chunk) {
+#pragma unroll 8
+                    for (int jj = 0; jj < kF32Chunk; ++jj) pair(tl[c0 + jj]);   // broadcast LDS.64
+                } else {
+                    for (int jj = 0; jj < m; ++jj) pair(tl[c0 + jj]);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    f0[r] += (double)sx[r];
+                    f1[r] += (double)sy[r];
+                }
+            }
+        });
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            if (i < N) {
+                partial0[(long long)slot * N + i] = pre * f0[r];
+                partial1[(long long)slot * N + i] = pre * f1[r];
+            }
+        }
+    }
+}
+
 // ---- potential-energy kernels (rows a-E2, a-E3) ---------------------------------------------------------
 // Full N x N sweep with the same partition; the j = i term is masked out; CTA k writes
 // vpart[k] = pre_half * sum over its ranges of sum_{i in tile} sum_{j in range, j != i} t_ij
@@ -273,9 +365,9 @@ __global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
 pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, double pre_half,
                    double* __restrict__ vpart) {
     constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
-    __shared__ PairSmem<TJ> sm;
+    __shared__ PairSmem<double2, TJ> sm;
     __shared__ double scratch[THREADS / 32];
-    JTilePipe<TJ> pipe(sm);
+    JTilePipe<double2, TJ> pipe(sm);
     pipe.init();
     const long long N = P.N;
     const double onepe = 1.0 + eps;
@@ -372,7 +464,8 @@ constexpr int kUpdThreads = 256;
 // js[i] = (cos th_i, sin th_i) (Ring; "computed and stored in global memory") or (x_i, y_i) (2D)
 template <int MODEL>
 __global__ void __launch_bounds__(kUpdThreads)
-pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, long long N, double2* __restrict__ js) {
+pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, long long N, double2* __restrict__ js,
+                 float2* __restrict__ js32) {
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
     if (MODEL == 1) {
@@ -381,6 +474,7 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
         js[i] = make_double2(c, s);
     } else {
         js[i] = make_double2(q0[i], q1[i]);
+        if (js32) js32[i] = make_float2((float)q0[i], (float)q1[i]);
     }
 }
 
@@ -397,7 +491,7 @@ template <int MODEL, bool KICK2, bool DRIFT>
 __global__ void __launch_bounds__(kUpdThreads)
 pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __restrict__ p0, double* __restrict__ p1,
                    PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
-                   double kickA, double kickB, double drift, double2* __restrict__ js) {
+                   double kickA, double kickB, double drift, double2* __restrict__ js, float2* __restrict__ js32) {
     const long long N = P.N;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
@@ -422,6 +516,7 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
             const double y = fma(drift, pb, q1[i]);
             q1[i] = y;
             js[i] = make_double2(x, y);
+            if (js32) js32[i] = make_float2((float)x, (float)y);
         } else {
             double sn, cs;
             sincos_any(x, sn, cs);

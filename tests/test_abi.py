@@ -82,11 +82,19 @@ def test_options(lrmd):
     assert lrmd.lrmd_set_option(h, lrmd.OPT_HMF_VARIANT, 1) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_VARIANT, 9999) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 2) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.EUNSUPPORTED   # fp32 pairs: GRAV2D only
     rc, b3 = lrmd.lrmd_workspace_bytes(h)
     lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, 32 * 6)
     rc, b6 = lrmd.lrmd_workspace_bytes(h)
     assert b6 > b3                                     # partial-force rows grow with the number of CTAs per tile
     assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)[1] in (6, 7)   # 6 equal ranges per tile, boundaries not tile-aligned
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(GRAV2D, 5000, 1e-3)
+    rc, b0 = lrmd.lrmd_workspace_bytes(h)
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.OK
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_PRECISION) == (lrmd.OK, 1)
+    rc, b1 = lrmd.lrmd_workspace_bytes(h)
+    assert b1 >= b0 + 5000 * 8                         # the fp32 copy of the positions
     lrmd.lrmd_destroy(h)
     rc, h = lrmd.lrmd_create(HMF, 50_000_000, 0.0)
     rc, g = lrmd.lrmd_get_option(h, lrmd.OPT_HMF_GRID)

@@ -354,6 +354,56 @@ def test_energy_any_partition(lrmd, ref, torch, S):
         assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
 
 
+# ---- fp32 pair arithmetic -----------------------------------------
+
+F32TOL = 1e-5    # north_star: 1e-5 * sum_j |f_ij| for the fp32 variant
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 255, 257, 1023, 4099, 20_011])
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_f32_pair_variant_forces(lrmd, ref, torch, N, variant):
+    """2D forces with fp32 pair terms summed in fp32 over <= 32 j, then in fp64 (reading G16), against the
+    fp64 oracle; odd j-range boundaries exercise the 16-byte alignment of the fp32 tile copies."""
+    st = _state(GRAV2D, N, 900 + N % 13)
+    f0, f1, A0, A1 = ref.forces_abs(GRAV2D, 1e-3, st[0], st[1], form=0)
+    for ctas in (0, 7):
+        got = _gpu_forces(lrmd, GRAV2D, 1e-3, st, options={lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_VARIANT: variant,
+                                                          lrmd.OPT_PAIR_CTAS: ctas})
+        for g, w, a in ((got[0], f0, A0), (got[1], f1, A1)):
+            err = np.abs(g - w)
+            assert np.all(err <= F32TOL * a + 1e-300), float((err / np.maximum(a, 1e-300)).max())
+
+
+def test_f32_pair_variant_is_not_the_fp64_path_and_is_reproducible(lrmd, ref, torch):
+    N = 6000
+    st = _state(GRAV2D, N, 4)
+    a = _gpu_forces(lrmd, GRAV2D, 1e-3, st, options={lrmd.OPT_PAIR_PRECISION: 1})
+    b = _gpu_forces(lrmd, GRAV2D, 1e-3, st, options={lrmd.OPT_PAIR_PRECISION: 1})
+    c = _gpu_forces(lrmd, GRAV2D, 1e-3, st)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    rel = np.max(np.abs(a[0] - c[0])) / np.max(np.abs(c[0]))
+    assert 1e-12 < rel < 1e-5       # differs from fp64 at the fp32 level, not more
+
+
+def test_f32_pair_variant_trajectory_and_energy(lrmd, ref, torch):
+    """10 steps with fp32 pair forces stay within 1e-6 of the fp64 oracle trajectory; the energies
+    (always fp64 kernels) match the oracle evaluated at the GPU's own final state."""
+    N = 3001
+    st = _state(GRAV2D, N, 21)
+    ctx = lrmd.Context(GRAV2D, N, 1e-3, options={lrmd.OPT_PAIR_PRECISION: 1})
+    ctx.set_state(*st)
+    ctx.step(10, 0.005)
+    got = ctx.state_numpy()
+    e = ctx.energy().cpu().numpy()
+    ctx.close()
+    r = [a.copy() for a in st]
+    ref.step(GRAV2D, 1e-3, r[0], r[1], r[2], r[3], 10, 0.005, form=1)
+    for g, w in zip(got, r):
+        assert np.max(np.abs(g - w)) <= 1e-6
+    er, ea = ref.energy(GRAV2D, 1e-3, got[0], got[1], got[2], got[3])
+    assert abs(e[0] - er[0]) <= 1e-12 * ea[0] and abs(e[1] - er[1]) <= 1e-12 * ea[1]
+
+
 # ---- integrator properties on the GPU ---------------------------------------------------------------
 
 @pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
