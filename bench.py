@@ -244,6 +244,25 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                      "traffic": NCU_TRAFFIC_BYTES.get(w.key)})
         out["roofline"] = roof
 
+    # ---- energy sums (rows a-E1..a-E3), timed apart from the steps
+    if w.key != "grav2d_1m":
+        ctx.energy()
+        torch.cuda.synchronize(dev)
+        ts = []
+        for _ in range(5):
+            if flush is not None:
+                flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            ctx.energy()
+            b.record(stream)
+            b.synchronize()
+            ts.append(a.elapsed_time(b))
+        ems = statistics.median(ts)
+        out["energy"] = {"ms_per_call": ems, "what": "lrmd_energy: K, V and momentum / magnetisation (3 launches)"}
+        if w.model != 0:
+            out["energy"]["pair_interactions_per_s"] = float(w.N) * float(w.N) / (ems * 1e-3)
+
     # ---- end to end through lrmd_step_host: pinned host buffers, copies inside the timed region
     if with_e2e:
         host = [torch.from_numpy(a.copy()).pin_memory() for a in st]
@@ -388,7 +407,7 @@ def main():
                    "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
                    "l2": res["l2"], "options": res["options"]},
         "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
-        "roofline": res.get("roofline"),
+        "roofline": res.get("roofline"), "energy": res.get("energy"),
     }
 
     if world == 1 and not args.only:
@@ -399,7 +418,7 @@ def main():
             ow = inputs.WORKLOADS[key]
             r = run_workload(ow, DEFAULT_STEPS[key], 3, None, with_e2e=(key != "grav2d_1m"))
             others[key] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options",
-                                              "clocks", "roofline", "e2e") if k in r}
+                                              "clocks", "roofline", "e2e", "energy") if k in r}
             others[key]["steps"] = DEFAULT_STEPS[key]
         # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
         r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)

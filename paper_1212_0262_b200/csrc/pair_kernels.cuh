@@ -21,6 +21,8 @@
 // (s_i c_i - c_i s_i evaluated with one FMA), which the epilogue removes again.
 #pragma once
 
+#include <type_traits>
+
 #include "common.cuh"
 #include "trig.cuh"
 
@@ -392,60 +394,67 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
             prod[r] = 1.0;
         }
         pipe.run(js, jbeg, jend, [&](const double2* tl, int cnt, long long j0) {
-            if (MODEL == 1) {
+            // only j-tiles that meet this i-tile's own rows can hold a j = i pair: they take the
+            // masked sweep, all others the plain one (no compare / select per pair)
+            const long long ilo = tile * CFG::ITILE;
+            const bool diag = (j0 < ilo + CFG::ITILE) && (j0 + cnt > ilo);
+            int jself[R];   // j - j0 of the row's own index (outside [0, cnt) if not in this tile)
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const long long dj = irow[r] - j0;
+                jself[r] = (dj >= 0 && dj < cnt) ? (int)dj : -1;
+            }
+            auto sweep = [&](auto masked) {
+                constexpr bool MASK = decltype(masked)::value;
+                if (MODEL == 1) {
 #pragma unroll 4
-                for (int jj = 0; jj < cnt; ++jj) {
-                    const double2 q = tl[jj];
+                    for (int jj = 0; jj < cnt; ++jj) {
+                        const double2 q = tl[jj];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const double d = fma(-b[r], q.y, fma(-a[r], q.x, onepe));
+                            const double y = rsqrt_refined(d);
+                            acc[r] += (MASK && jself[r] == jj) ? 0.0 : y;
+                        }
+                    }
+                } else {
+                    int esum[R];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) esum[r] = 0;
+                    for (int jb = 0; jb < cnt; jb += 8) {
+                        const int m = (cnt - jb < 8) ? (cnt - jb) : 8;
+                        auto one = [&](int jj) {
+                            const double2 q = tl[jj];
+#pragma unroll
+                            for (int r = 0; r < R; ++r) {
+                                const double dx = a[r] - q.x, dy = b[r] - q.y;
+                                double d = fma(dy, dy, fma(dx, dx, eps));
+                                if (MASK) d = (jself[r] == jj) ? 1.0 : d;
+                                prod[r] *= d;
+                            }
+                        };
+                        if (m == 8) {
+#pragma unroll
+                            for (int u = 0; u < 8; ++u) one(jb + u);
+                        } else {
+                            for (int u = 0; u < m; ++u) one(jb + u);
+                        }
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {   // move the exponent into the integer counter
+                            const int hi = __double2hiint(prod[r]);
+                            esum[r] += ((hi >> 20) & 0x7ff) - 1023;
+                            prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
+                        }
+                    }
 #pragma unroll
                     for (int r = 0; r < R; ++r) {
-                        const double d = fma(-b[r], q.y, fma(-a[r], q.x, onepe));
-                        const double y = rsqrt_refined(d);
-                        acc[r] += (irow[r] == j0 + jj) ? 0.0 : y;
+                        acc[r] += fma((double)esum[r], kLn2, log(prod[r]));
+                        prod[r] = 1.0;
                     }
                 }
-            } else {
-                int esum[R];
-#pragma unroll
-                for (int r = 0; r < R; ++r) esum[r] = 0;
-                for (int jb = 0; jb < cnt; jb += 8) {
-                    const int m = (cnt - jb < 8) ? (cnt - jb) : 8;
-                    if (m == 8) {
-#pragma unroll
-                        for (int u = 0; u < 8; ++u) {
-                            const double2 q = tl[jb + u];
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double dx = a[r] - q.x, dy = b[r] - q.y;
-                                double d = fma(dy, dy, fma(dx, dx, eps));
-                                d = (irow[r] == j0 + jb + u) ? 1.0 : d;
-                                prod[r] *= d;
-                            }
-                        }
-                    } else {
-                        for (int u = 0; u < m; ++u) {
-                            const double2 q = tl[jb + u];
-#pragma unroll
-                            for (int r = 0; r < R; ++r) {
-                                const double dx = a[r] - q.x, dy = b[r] - q.y;
-                                double d = fma(dy, dy, fma(dx, dx, eps));
-                                d = (irow[r] == j0 + jb + u) ? 1.0 : d;
-                                prod[r] *= d;
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {   // move the exponent into the integer counter
-                        const int hi = __double2hiint(prod[r]);
-                        esum[r] += ((hi >> 20) & 0x7ff) - 1023;
-                        prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
-                    }
-                }
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    acc[r] += fma((double)esum[r], kLn2, log(prod[r]));
-                    prod[r] = 1.0;
-                }
-            }
+            };
+            if (diag) sweep(std::true_type{});
+            else sweep(std::false_type{});
         });
 #pragma unroll
         for (int r = 0; r < R; ++r)
