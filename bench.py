@@ -45,8 +45,12 @@ PAIR_FP64_INSTR = {1: 11.0, 2: 9.0}
 HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` captures (profiles/*.md name the command); None = not captured yet.
-NCU_TRAFFIC_BYTES = {"ring_16k": None, "grav2d_64k": None, "hmf_5e7": None, "grav2d_1m": None, "hmf_1e4": None}
+# `ncu --set full` captures (profiles/r01d_summary.md names the commands); None = not captured.
+# hmf_5e7: 800.0 MB read + 741.7 MB written of 1600 MB algorithmic (the last lines written are still in L2
+# when the kernel ends); the pair kernels read the 16 N (8 N for fp32) byte j-stream once from DRAM, the
+# tiles' re-reads hit L2.
+NCU_TRAFFIC_BYTES = {"ring_16k": 279808.0, "grav2d_64k": 1067264.0, "hmf_5e7": 1541759232.0, "grav2d_1m": None,
+                     "hmf_1e4": None, "grav2d_64k_f32": 554240.0}
 
 DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5}
 
@@ -241,7 +245,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         roof.update({"kernel": "hmf_substage_kernel" if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else "pair_force_kernel"),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
-                     "traffic": NCU_TRAFFIC_BYTES.get(w.key)})
+                     "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else ""))})
         out["roofline"] = roof
 
     # ---- energy sums (rows a-E1..a-E3), timed apart from the steps
