@@ -118,6 +118,23 @@ class ClockSampler:
         }
 
 
+# ---- replicas over ranks (the path does not shard; no data-path collective) -----------
+
+def max_over_ranks(x: float, dist_mod, device) -> float:
+    """MAX of a per-rank scalar over all ranks (the only collective bench.py uses: timing, not data)."""
+    if dist_mod is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist_mod.all_reduce(t, op=dist_mod.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_rank_step: float, steps: int, ms_max: float, world: int) -> float:
+    """Aggregate throughput of `world` independent replicas: all units processed / slowest rank's device time."""
+    return world * units_per_rank_step * steps / (ms_max * 1e-3)
+
+
 # ---- one workload on this rank's GPU ------------------------------------------------------------------------
 
 def units_per_force(w):
@@ -179,21 +196,15 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     launches = ctx.launch_count() - l0
     barrier()
     clocks = sampler.stop()
-    ms_max = ms
-    world = 1
-    if dist_ctx is not None:
-        import torch.distributed as dist
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_max = float(t.item())
-        world = dist.get_world_size()
+    ms_max = max_over_ranks(ms, dist_ctx, dev)
+    world = dist_ctx.get_world_size() if dist_ctx is not None else 1
 
     metric, unit, upf = units_per_force(w)
     if w.model == 0:
         units_per_step = float(w.N)
     else:
         units_per_step = 3.0 * upf
-    value = world * units_per_step * K / (ms_max * 1e-3)
+    value = whole_job_value(units_per_step, K, ms_max, world)
 
     out = {
         "metric": metric, "value": value, "unit": unit, "ms_per_step": ms_max / K,
@@ -279,11 +290,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         ctx.step_host(host, Ke, w.dt)                         # synchronises the stream before returning
         t1 = time.perf_counter()
         dt_s = t1 - t0
-        if dist_ctx is not None:
-            import torch.distributed as dist
-            t = torch.tensor([dt_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt_s = float(t.item())
+        dt_s = max_over_ranks(dt_s, dist_ctx, dev)
         if w.model == 0:
             e_units = float(w.N) * Ke
         else:

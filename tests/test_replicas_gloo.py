@@ -1,0 +1,74 @@
+"""Multi-rank host logic of bench.py on CPU (gloo, world_size 2).  The hot path does not shard
+(BASELINE.json north_star: one GPU, no sharding or collectives; replicas only), so the
+only multi-rank logic is: barrier, MAX of the per-rank device time, whole-job value = all ranks' units /
+slowest rank's time; `--impl reference` runs on rank 0 only."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms_local = 10.0 + 5.0 * rank                      # rank 1 is the slow replica
+    dist.barrier()
+    ms_max = bench.max_over_ranks(ms_local, dist, torch.device("cpu"))
+    value = bench.whole_job_value(1000.0, 4, ms_max, dist.get_world_size())
+    out[rank] = (ms_max, value)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_max_over_ranks_and_whole_job_value_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    with ctx.Manager() as m:
+        out = m.dict()
+        port = 29500 + os.getpid() % 1000
+        procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+        for p in procs:
+            p.start()
+        for p in procs:
+            p.join(120)
+            assert p.exitcode == 0
+        res = dict(out)
+    # both ranks see the slowest replica's time; 2 replicas x 1000 units x 4 steps / 15 ms
+    for r in (0, 1):
+        assert res[r][0] == 15.0
+        assert abs(res[r][1] - 2 * 1000.0 * 4 / 15e-3) < 1e-6
+
+
+def test_single_rank_needs_no_process_group():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks(3.5, None, None) == 3.5
+    assert bench.whole_job_value(10.0, 2, 4.0, 1) == 10.0 * 2 / 4e-3
+
+
+def test_reference_arm_runs_on_rank0_only():
+    """Under torchrun the oracle arm prints on rank 0; other ranks exit 0 without work or output."""
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+@pytest.mark.parametrize("workload", ["hmf_1e4"])
+def test_reference_arm_line_rank0(workload):
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", workload,
+                        "--steps", "1", "--warmup", "0"], capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "particle-steps/s"
