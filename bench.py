@@ -230,6 +230,10 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         clk = (clocks.get("sm_mhz") or peaks["sm_max_mhz"])
         if w.model == 0:
             bytes_per_launch = HMF_BYTES_PER_PARTICLE_SUBSTAGE * w.N
+            if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3:
+                # cluster-resident kernel: one launch runs all Kr steps with the state in registers; the figure is
+                # what the same substages would stream through HBM (context only: the working set is on chip)
+                bytes_per_launch *= 3.0 * Kr
             achieved = bytes_per_launch / avg_s / 1e9
             roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
@@ -253,7 +257,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                     "algorithmic_flop_per_launch": flop,
                     "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
                     "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
-        roof.update({"kernel": "hmf_substage_kernel" if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else "pair_force_kernel"),
+        roof.update({"kernel": ("hmf_cluster_kernel" if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3 else "hmf_substage_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else "pair_force_kernel"),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else ""))})

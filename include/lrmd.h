@@ -69,8 +69,9 @@ enum {
                                     substage kernel; RING/GRAV2D: the pair-force kernel) with a CUDA event
                                     pair on the launching stream; read with lrmd_kernel_time.  Turns CUDA-graph
                                     replay off while set.  Measurement aid: results are unchanged.          */
-    LRMD_OPT_HMF_VARIANT = 5,    /* HMF: launch shape of the fused substage kernel: 0 = register-prefetch
-                                    kernel, >= 1 = TMA-staged kernel shapes (-1 = choose from N)              */
+    LRMD_OPT_HMF_VARIANT = 5,    /* HMF: 0 = register-prefetch substage kernel, 1-2 = TMA-staged substage kernel
+                                    shapes, 3 = cluster-resident kernel (N <= 20,480: state in registers of one
+                                    thread-block cluster, all n steps of a call in one launch); -1 = choose from N */
     LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
                                     of the pair kernels (-1 = choose)                                          */
     LRMD_OPT_PAIR_SLOTS = 7      /* read-only (lrmd_get_option): partial force rows per particle          */

@@ -303,6 +303,128 @@ hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long
     }
 }
 
+// ---- cluster-resident variant (small N: the step is latency-bound, SURVEY.md hard part 4) ---------------
+// One thread-block cluster of kHmfClusterCtas CTAs holds the whole state in registers (P particles
+// per thread) and runs ALL n steps of an lrmd_step call in one launch: 3n + 1 reductions, each
+//   per-thread sum -> warp shuffle tree -> shared memory -> warp 0 -> the CTA's (sum cos, sum sin)
+//   written into every CTA's shared memory (distributed shared memory, st.shared::cluster)
+//   -> barrier.cluster arrive.release / wait.acquire -> every thread adds the C partials in rank order,
+// so a substage costs one CTA barrier and one cluster barrier instead of a kernel boundary.  sin / cos
+// of the current angles stay in registers from the reduction to the next kick (one sincos per
+// particle-substage instead of two).  Deterministic: fixed particle -> thread map, fixed trees.
+constexpr int kHmfClusterCtas = 8;      // portable cluster size
+constexpr int kHmfClusterCtasMax = 16;  // non-portable size, used when the device grants it
+constexpr int kHmfClusterThreads = 640;
+
+__device__ __forceinline__ unsigned cluster_ctarank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ unsigned cluster_nctarank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// store (a, b) at the address of `local` in CTA `rank` of the cluster
+__device__ __forceinline__ void dsmem_store2(double2* local, unsigned rank, double a, double b) {
+    unsigned remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(local)), "r"(rank));
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(remote), "d"(a), "d"(b) : "memory");
+}
+
+template <int P>
+__global__ void __launch_bounds__(kHmfClusterThreads, 1)
+hmf_cluster_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, long long nsteps, double kB0,
+                   double kB1, double dD0, double dD1, double2* __restrict__ partial_out) {
+    constexpr int T = kHmfClusterThreads, NW = T / 32;
+    __shared__ double2 warp_part[NW];
+    __shared__ double2 cta_part[2][kHmfClusterCtasMax];      // [parity][rank of the writer]
+    const int C = (int)cluster_nctarank();  // 8 or 16 CTAs
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const unsigned rank = cluster_ctarank();
+    const double inv_n = 1.0 / (double)N;
+
+    double th[P], pp[P], sn[P], cs[P];
+    bool valid[P];
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        const long long i = (long long)k * (C * T) + (long long)rank * T + tid;
+        valid[k] = i < N;
+        th[k] = valid[k] ? theta[i] : 0.0;
+        pp[k] = valid[k] ? p[i] : 0.0;
+    }
+    cluster_sync_all();     // every CTA of the cluster is running before the first remote store
+
+    int parity = 0;
+    double Mx = 0.0, My = 0.0;
+    auto reduce = [&]() {
+        bool small = true;
+#pragma unroll
+        for (int k = 0; k < P; ++k) small = small && sincos_is_small(th[k]);
+        if (small) {
+#pragma unroll
+            for (int k = 0; k < P; ++k) sincos_fast(th[k], sn[k], cs[k]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < P; ++k) {
+                const double2 r = sincos_any_call(th[k]);
+                sn[k] = r.x;
+                cs[k] = r.y;
+            }
+        }
+        double aC = 0.0, aS = 0.0;
+#pragma unroll
+        for (int k = 0; k < P; ++k)
+            if (valid[k]) { aC += cs[k]; aS += sn[k]; }
+        aC = warp_sum(aC);
+        aS = warp_sum(aS);
+        if (lane == 0) warp_part[w] = make_double2(aC, aS);
+        __syncthreads();
+        if (w == 0) {
+            const double2 q = (lane < NW) ? warp_part[lane] : make_double2(0.0, 0.0);
+            const double tC = warp_sum(q.x), tS = warp_sum(q.y);
+            if (lane < C) dsmem_store2(&cta_part[parity][rank], (unsigned)lane, tC, tS);
+        }
+        cluster_sync_all();
+        double sC = 0.0, sS = 0.0;
+        for (int r = 0; r < C; ++r) {
+            const double2 q = cta_part[parity][r];
+            sC += q.x;
+            sS += q.y;
+        }
+        Mx = sC * inv_n;
+        My = sS * inv_n;
+        parity ^= 1;
+    };
+    auto kick = [&](double kc) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) pp[k] = fma(kc, fma(cs[k], My, -(sn[k] * Mx)), pp[k]);
+    };
+    auto drift = [&](double dc) {
+#pragma unroll
+        for (int k = 0; k < P; ++k) th[k] = fma(dc, pp[k], th[k]);
+    };
+
+    reduce();                                   // f(q(t)): listing step 1
+    for (long long s = 0; s < nsteps; ++s) {    // listing steps 2-11, readings G2-G4
+        kick(kB0); drift(dD0); reduce();
+        kick(kB1); drift(dD1); reduce();
+        kick(kB1); drift(dD0); reduce();
+        kick(kB0);
+    }
+#pragma unroll
+    for (int k = 0; k < P; ++k) {
+        const long long i = (long long)k * (C * T) + (long long)rank * T + tid;
+        if (valid[k]) { theta[i] = th[k]; p[i] = pp[k]; }
+    }
+    // the sums at the final angles, for lrmd_forces / lrmd_energy / the next call (reading G3)
+    if (rank == 0 && tid < C) partial_out[tid] = cta_part[parity ^ 1][tid];
+}
+
 // f_i = cos(theta_i) My - sin(theta_i) Mx  -> f   (lrmd_forces; eq.(6))
 __global__ void __launch_bounds__(kHmfThreads)
 hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long long N,

@@ -80,10 +80,12 @@ namespace {
 // ---- option resolution -------------------------------------------------------------------------------
 
 // Launch shapes compiled in (chosen from sweeps on B200, profiles/r01_sweeps.md).
-// HMF: variant 0 is the register-prefetch kernel (best below ~1e6 particles, where the step is latency
-// bound), the others the TMA-staged kernel <consumer threads, stages, CTAs per SM>.
+// HMF: variant 0 is the register-prefetch kernel, 1-2 the TMA-staged kernel <consumer threads, stages, CTAs per
+// SM> (N >= 1e6), 3 the cluster-resident kernel (N <= 20,480: the step is latency-bound).
 struct HmfVariant { int consumers, stages, minb; };
-constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}};
+constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}, {-1, 0, 0}};
+constexpr int kHmfClusterVariant = 3;   // cluster-resident kernel: whole state in registers, all steps in one launch
+constexpr int64_t kHmfClusterMaxN = (int64_t)kHmfClusterCtas * kHmfClusterThreads * 4;   // 20,480
 constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
 constexpr int64_t kHmfTmaMinN = 1000000;
 
@@ -107,10 +109,15 @@ void resolve(lrmd_ctx* c) {
     Layout L;
     size_t off = 0;
     if (c->model == LRMD_HMF) {
-        c->hmf_variant = c->opt_hmf_variant >= 0 ? (int)c->opt_hmf_variant : (N >= kHmfTmaMinN ? 1 : 0);
+        c->hmf_variant = c->opt_hmf_variant >= 0 ? (int)c->opt_hmf_variant
+                         : (N >= kHmfTmaMinN ? 1 : (N <= kHmfClusterMaxN ? kHmfClusterVariant : 0));
+        if (c->hmf_variant == kHmfClusterVariant && N > kHmfClusterMaxN) c->hmf_variant = 0;
         const HmfVariant hv = kHmfVariants[c->hmf_variant];
         int64_t g;
-        if (c->hmf_variant == 0) {
+        if (c->hmf_variant == kHmfClusterVariant) {
+            // the other HMF kernels of this context (forces, energy) read this many partials
+            g = c->opt_hmf_grid == kHmfClusterCtasMax ? kHmfClusterCtasMax : kHmfClusterCtas;
+        } else if (c->hmf_variant == 0) {
             const int64_t nvec = N >> 2;
             g = c->opt_hmf_grid > 0 ? c->opt_hmf_grid : (nvec + kHmfThreads - 1) / kHmfThreads;
         } else {
@@ -125,6 +132,7 @@ void resolve(lrmd_ctx* c) {
         c->slots = 1;
         L.hmf_partial = off; off = align_up(off + 3 * sizeof(double2) * kHmfMaxGrid);
         c->use_graph = c->opt_graph < 0 ? (N <= (1 << 20)) : (c->opt_graph != 0);
+        if (c->hmf_variant == kHmfClusterVariant) c->use_graph = false;
     } else {
         c->pair_variant = c->opt_pair_variant >= 0 ? (int)c->opt_pair_variant : (c->model == LRMD_GRAV2D ? 1 : 0);
         int itile = 0, minb = 0;
@@ -352,7 +360,56 @@ int hmf_build_graph(lrmd_ctx* c, const Coef& k, double dt) {
     return rc;
 }
 
+// All n steps in one launch of one thread-block cluster (hmf_cluster_kernel).
+int hmf_step_cluster(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
+    const Coef k = coefficients();
+    const int ctas = c->hmf_grid;     // 8, or 16 when the device grants the non-portable cluster size
+    const int64_t per = (int64_t)ctas * kHmfClusterThreads;
+    const int P = c->N <= per ? 1 : (c->N <= 2 * per ? 2 : 4);
+    void (*kernel)(double*, double*, long long, long long, double, double, double, double, double2*) =
+        P == 1 ? hmf_cluster_kernel<1> : (P == 2 ? hmf_cluster_kernel<2> : hmf_cluster_kernel<4>);
+    if (ctas > kHmfClusterCtas) {
+        bool ready = false;
+        for (const void* f : c->smem_ready) ready = ready || f == (const void*)kernel;
+        if (!ready) {
+            const cudaError_t ea = cudaFuncSetAttribute((const void*)kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (ea != cudaSuccess) { c->cuda_err = (int)ea; (void)cudaGetLastError(); return LRMD_ECUDA; }
+            c->smem_ready.push_back((const void*)kernel);
+        }
+    }
+    cudaLaunchConfig_t cfg;
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(ctas);
+    cfg.blockDim = dim3(kHmfClusterThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = ctas;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const bool t = c->timing && c->ev_used + 2 <= kMaxTimedEvents;
+    if (t) {
+        while (c->ev.size() < c->ev_used + 2) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); return LRMD_ECUDA; }
+            c->ev.push_back(e);
+        }
+        cudaEventRecord(c->ev[c->ev_used], stream);
+    }
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, c->a0, c->a1, (long long)c->N, (long long)n, k.B0 * dt,
+                                             k.B1 * dt, k.D0 * dt, k.D1 * dt, hmf_buf(c, c->cur));
+    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_ECUDA; }
+    if (t) { cudaEventRecord(c->ev[c->ev_used + 1], stream); c->ev_used += 2; }
+    ++c->launches;
+    c->force_valid = true;   // the kernel leaves the sums at the final angles in the current partial buffer
+    return LRMD_OK;
+}
+
 int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
+    if (c->hmf_variant == kHmfClusterVariant) return hmf_step_cluster(c, n, dt, stream);
     const Coef k = coefficients();
     Launcher L{c, stream};
     if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }

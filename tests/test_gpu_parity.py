@@ -131,6 +131,58 @@ def test_hmf_tma_variants_match_oracle(lrmd, ref, torch, variant, N):
     assert abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N) + 1e-300
 
 
+@pytest.mark.parametrize("N", [1, 2, 31, 640, 5119, 5120, 5121, 10_000, 10_241, 20_480])
+def test_hmf_cluster_resident_kernel_matches_oracle(lrmd, ref, torch, N):
+    """Cluster-resident HMF kernel (variant 3; 1, 2 or 4 particles per thread): 7-step trajectory, the
+    cached sums it leaves behind (forces, energy) and step(n) == n x step(1) bit for bit."""
+    st = _state(HMF, N, 300 + N % 11)
+    ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: 3})
+    assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3
+    ctx.set_state(*st)
+    ctx.step(7, 0.05)
+    out = ctx.state_numpy()
+    f = ctx.forces().cpu().numpy()
+    e = ctx.energy().cpu().numpy()
+    assert ctx.launch_count() <= 1 + 1 + 2      # one launch for the 7 steps, one for forces, two for the energy
+    ctx.close()
+    th, p = st[0].copy(), st[1].copy()
+    ref.step(HMF, 0.0, th, None, p, None, 7, 0.05, form=0)
+    assert np.max(np.abs(out[0] - th)) <= XTOL and np.max(np.abs(out[1] - p)) <= XTOL
+    f0, _, S0, _ = ref.forces_abs(HMF, 0.0, out[0], None, form=0)      # at the GPU's own final angles
+    assert np.all(np.abs(f - f0) <= FTOL * S0 + 4e-16)
+    er, ea = ref.energy(HMF, 0.0, out[0], None, out[1], None)
+    assert abs(e[0] - er[0]) <= 1e-12 * ea[0] + 1e-300 and abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N) + 1e-300
+    b = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: 3})
+    b.set_state(*st)
+    for _ in range(7):
+        b.step(1, 0.05)
+    for x, y in zip(out, b.state_numpy()):
+        assert np.array_equal(x, y)
+    b.close()
+
+
+def test_hmf_cluster_of_16_ctas_same_trajectory(lrmd, torch):
+    """The non-portable cluster size (LRMD_OPT_HMF_GRID = 16) changes the summation tree only."""
+    N = 10_000
+    st = _state(HMF, N, 77)
+    outs = []
+    for g in (8, 16):
+        ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: 3, lrmd.OPT_HMF_GRID: g})
+        ctx.set_state(*st)
+        ctx.step(25, 0.05)
+        assert ctx.get_option(lrmd.OPT_HMF_GRID) == g
+        outs.append(ctx.state_numpy())
+        ctx.close()
+    for x, y in zip(*outs):
+        assert np.max(np.abs(x - y)) <= 1e-11
+
+
+def test_hmf_cluster_variant_falls_back_above_its_size(lrmd, torch):
+    ctx = lrmd.Context(HMF, 20_481, 0.0, options={lrmd.OPT_HMF_VARIANT: 3})
+    assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == 0
+    ctx.close()
+
+
 @pytest.mark.parametrize("variant", [1, 2])
 def test_hmf_tma_variant_graph_and_grid(lrmd, torch, variant):
     """Graph replay and a non-default grid give the same bits as plain launches of the same variant and grid."""
