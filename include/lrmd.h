@@ -119,6 +119,14 @@ int lrmd_forces(lrmd_ctx* ctx, double* f0, double* f1, void* cuda_stream);
  *   (a, b) = (Mx, My) for HMF, (sum p, 0) for RING, (sum px, sum py) for GRAV2D. */
 int lrmd_energy(lrmd_ctx* ctx, double* out4_device, void* cuda_stream);
 
+/* Advance n >= 0 steps and record the observables the paper plots against time (K, V and the energy
+ * error derived from them, PAPER.md:136 and Figs. 3-6; "compute any properties of interest", listing
+ * step 12): out_device (DEVICE pointer, 4 * (n / every + 1) doubles) receives the
+ * lrmd_energy record {K, V, a, b} of the initial state followed by one record after every `every`-th
+ * step (every >= 1).  Steps left over after the last record (n % every) are taken without a record.
+ * Asynchronous on the stream, like lrmd_step. */
+int lrmd_step_observe(lrmd_ctx* ctx, int64_t n, double dt, int64_t every, double* out_device, void* cuda_stream);
+
 /* Set an option (keys above).  Unknown key or bad value: LRMD_EINVAL. */
 int lrmd_set_option(lrmd_ctx* ctx, int key, int64_t value);
 /* Read back an option as resolved for this context (e.g. the j-split chosen from N). */

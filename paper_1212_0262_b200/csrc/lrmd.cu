@@ -670,6 +670,22 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
     return L.rc;
 }
 
+int lrmd_step_observe(lrmd_ctx* c, int64_t n, double dt, int64_t every, double* out_device, void* cuda_stream) {
+    int rc = ready(c);
+    if (rc != LRMD_OK) return rc;
+    if (n < 0 || every < 1 || !std::isfinite(dt) || !out_device) return LRMD_EINVAL;
+    rc = lrmd_energy(c, out_device, cuda_stream);
+    int64_t done = 0, rec = 1;
+    while (rc == LRMD_OK && done + every <= n) {
+        rc = lrmd_step(c, every, dt, cuda_stream);
+        if (rc == LRMD_OK) rc = lrmd_energy(c, out_device + 4 * rec, cuda_stream);
+        done += every;
+        ++rec;
+    }
+    if (rc == LRMD_OK && done < n) rc = lrmd_step(c, n - done, dt, cuda_stream);
+    return rc;
+}
+
 int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
     if (!c) return LRMD_EINVAL;
     switch (key) {

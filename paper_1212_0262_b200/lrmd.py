@@ -25,7 +25,7 @@ SYMBOLS = (
     "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
-    "lrmd_pair_partition",
+    "lrmd_pair_partition", "lrmd_step_observe",
 )
 
 _lib = None
@@ -76,6 +76,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_coefficients.argtypes = [C.POINTER(_dbl)]
     lib.lrmd_host_sincos.argtypes = [_vp, _i64, _vp, _vp]
     lib.lrmd_pair_partition.argtypes = [_vp, _i64, _vp, _i64, C.POINTER(_i64)]
+    lib.lrmd_step_observe.argtypes = [_vp, _i64, _dbl, _i64, _vp, _vp]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int
@@ -113,6 +114,10 @@ def lrmd_set_state(ctx, a0: int, a1: int, a2: int | None = None, a3: int | None 
 
 def lrmd_step(ctx, n: int, dt: float, stream: int = 0):
     return load().lrmd_step(ctx, int(n), float(dt), stream)
+
+
+def lrmd_step_observe(ctx, n: int, dt: float, every: int, out_device: int, stream: int = 0):
+    return load().lrmd_step_observe(ctx, int(n), float(dt), int(every), out_device, stream)
 
 
 def lrmd_step_host(ctx, h0: int, h1: int, h2: int | None, h3: int | None, n: int, dt: float, stream: int = 0):
@@ -281,6 +286,15 @@ class Context:
     def step(self, n: int, dt: float, stream=None):
         with self._torch.cuda.device(self.device):
             self._chk(lrmd_step(self._h, n, dt, self._stream(stream)), "lrmd_step")
+
+    def step_observe(self, n: int, dt: float, every: int = 1, stream=None):
+        """``n`` steps with an ``lrmd_energy`` record {K, V, a, b} of the initial state and after every
+        ``every``-th step: returns a device tensor of shape (n // every + 1, 4)."""
+        torch = self._torch
+        out = torch.empty((n // every + 1, 4), dtype=torch.float64, device=self.device)
+        with torch.cuda.device(self.device):
+            self._chk(lrmd_step_observe(self._h, n, dt, every, out.data_ptr(), self._stream(stream)), "lrmd_step_observe")
+        return out
 
     def step_host(self, host_arrays, n: int, dt: float, stream=None):
         """End to end through ``lrmd_step_host``: ``host_arrays`` are (pinned) CPU fp64 tensors,

@@ -637,3 +637,41 @@ def test_negative_n_and_nonfinite_dt_rejected(lrmd, torch):
     ctx.step(0, 0.1)
     assert all(np.array_equal(a, b) for a, b in zip(before, ctx.state_numpy()))
     ctx.close()
+
+
+# ---- per-step observables and paper-shaped runs (Figs. 3-6) --------------
+
+@pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
+def test_step_observe_records_match_oracle(lrmd, ref, torch, model):
+    """lrmd_step_observe: K(t), V(t) records every 3 steps against the oracle stepped alongside."""
+    eps = _eps(model)
+    N = 1500
+    st = _state(model, N, 61)
+    ctx = lrmd.Context(model, N, eps)
+    ctx.set_state(*st)
+    rec = ctx.step_observe(10, 0.01, 3).cpu().numpy()          # records at steps 0, 3, 6, 9; 10 steps taken
+    fin = ctx.state_numpy()
+    ctx.close()
+    assert rec.shape == (4, 4)
+    r = [a.copy() for a in st]
+    q0, q1 = _q(model, r)
+    p0, p1 = _p(model, r)
+    f0 = f1 = None
+    for k in range(4):
+        er, ea = ref.energy(model, eps, q0, q1, p0, p1)
+        assert abs(rec[k, 0] - er[0]) <= 1e-9 * max(ea[0], 1e-300) and abs(rec[k, 1] - er[1]) <= 1e-9 * max(ea[1], 0.5 * N)
+        f0, f1 = ref.step(model, eps, q0, q1, p0, p1, 3 if k < 3 else 1, 0.01, f0, f1, force_valid=(k > 0), form=(0 if model == HMF else 1))
+    for g, w in zip(fin, r):
+        assert np.max(np.abs(g - w)) <= XTOL
+
+
+def test_paper_shaped_runs_conserve_energy(lrmd, torch):
+    """homogeneous state at rest (HMF dt = 0.1; Ring eps = 1e-3, dt = 0.005) and the 2D annulus
+    1.0 <= r <= 1.5 at rest: K starts at 0, grows as the system collapses / relaxes, the relative energy
+    error stays at the 4th-order level."""
+    from paper_1212_0262_b200 import paper_runs
+    for name, n, tol in (("hmf", 20_000, 1e-5), ("ring", 4096, 1e-4), ("grav2d", 4096, 1e-6)):
+        out = paper_runs.run(name, n, steps=60, every=10)
+        assert out["K"][0] == 0.0 and len(out["K"]) == 7
+        assert out["K"][-1] > 0.0
+        assert max(out["energy_error"]) < tol, (name, max(out["energy_error"]))
