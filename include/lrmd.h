@@ -53,7 +53,8 @@ enum {
     LRMD_EINVAL = -1,        /* bad argument (NULL, wrong NULL pattern, N < 1, eps <= 0 ...)  */
     LRMD_ESTATE = -2,        /* state or workspace not set                                     */
     LRMD_ECUDA = -3,         /* a CUDA call failed; see lrmd_last_cuda_error                   */
-    LRMD_EUNSUPPORTED = -4   /* valid request this build does not implement                    */
+    LRMD_EUNSUPPORTED = -4,  /* valid request this build does not implement                    */
+    LRMD_ECOLL = -5          /* a collective callback of a sharded context returned non-zero   */
 };
 
 /* lrmd_set_option keys */
@@ -126,6 +127,26 @@ int lrmd_energy(lrmd_ctx* ctx, double* out4_device, void* cuda_stream);
  * step (every >= 1).  Steps left over after the last record (n % every) are taken without a record.
  * Asynchronous on the stream, like lrmd_step. */
 int lrmd_step_observe(lrmd_ctx* ctx, int64_t n, double dt, int64_t every, double* out_device, void* cuda_stream);
+
+/* Multi-GPU sharding (PAPER.md:82 for HMF, PAPER.md:112-124 for the pair models).  One process
+ * per GPU; each creates its context with N = the number of particles it OWNS and declares here that they are the
+ * global indices i0 .. i0 + N - 1 of N_total.  State arrays, forces and lrmd_step_host buffers hold the owned
+ * particles only.  The exchange steps are the caller's collectives (NCCL through torch.distributed in the Python
+ * binding), called by the library on the stream between its kernels:
+ *   HMF          after every reduction: allreduce(device pointer to this rank's (sum cos, sum sin), 2, stream, user)
+ *                must sum the 2 doubles over all ranks in place ("each GPU computes its contribution to the
+ *                magnetisation, which are then summed");
+ *   RING/GRAV2D  after every drift: allgather(device pointer to the packed j-stream of ALL N_total particles,
+ *                elem_bytes, i0, N, N_total, stream, user) — this rank's N elements are already in place at element
+ *                offset i0; the callback must fill in the other ranks' ("each GPU holds all positions").
+ * A callback returns 0 on success.  lrmd_energy on a shard returns this rank's part of K, of V (pair models: rows
+ * owned x all j, halved) and of the momentum sums — add them over ranks; HMF's V, Mx, My are already global.
+ * N_total = N (a single shard) restores the unsharded path.  Changes the workspace size. */
+typedef int (*lrmd_allreduce_fn)(void* device_doubles, int64_t count, void* cuda_stream, void* user);
+typedef int (*lrmd_allgather_fn)(void* device_all, int64_t elem_bytes, int64_t i0, int64_t n_local, int64_t n_total,
+                                 void* cuda_stream, void* user);
+int lrmd_set_shard(lrmd_ctx* ctx, int64_t N_total, int64_t i0, lrmd_allreduce_fn allreduce, lrmd_allgather_fn allgather,
+                   void* user);
 
 /* Set an option (keys above).  Unknown key or bad value: LRMD_EINVAL. */
 int lrmd_set_option(lrmd_ctx* ctx, int key, int64_t value);

@@ -118,8 +118,9 @@ __device__ __forceinline__ void hmf_particle(double& th, double& p, double Mx, d
 // DRIFT: theta += drift p.   REDUCE: write per-CTA (sum cos, sum sin) of the final angles.
 template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
 __global__ void __launch_bounds__(kHmfThreads)
-hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double kickA, double kickB,
-                    double drift, const double2* __restrict__ partial_in, int g_in, double2* __restrict__ partial_out) {
+hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double inv_n, double kickA,
+                    double kickB, double drift, const double2* __restrict__ partial_in, int g_in,
+                    double2* __restrict__ partial_out) {
     __shared__ double scratch[2 * (kHmfThreads / 32)];
     const long long nvec = N >> 2;
     const long long stride = (long long)gridDim.x * kHmfThreads;
@@ -133,7 +134,7 @@ hmf_substage_kernel(double* __restrict__ theta, double* __restrict__ p, long lon
         if (KICK || DRIFT) p4 = ld256(p + 4 * v);
     }
     double Mx = 0.0, My = 0.0;
-    if (KICK) hmf_magnetisation<kHmfThreads>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+    if (KICK) hmf_magnetisation<kHmfThreads>(partial_in, g_in, inv_n, scratch, Mx, My);
 
     double accC = 0.0, accS = 0.0;
     while (v < nvec) {
@@ -191,8 +192,8 @@ struct HmfTma {
 
 template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE, int CONSUMERS, int NS, int MINB>
 __global__ void __launch_bounds__(CONSUMERS + 32, MINB)
-hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double kickA, double kickB,
-                        double drift, const double2* __restrict__ partial_in, int g_in,
+hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, double inv_n, double kickA,
+                        double kickB, double drift, const double2* __restrict__ partial_in, int g_in,
                         double2* __restrict__ partial_out) {
     using Cfg = HmfTma<CONSUMERS, NS>;
     constexpr int C = Cfg::kChunk;
@@ -235,7 +236,7 @@ hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long
         for (int k = 0; k < NS && k < nmine; ++k) issue_load(k);
 
     double Mx = 0.0, My = 0.0;
-    if (KICK) hmf_magnetisation<T>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+    if (KICK) hmf_magnetisation<T>(partial_in, g_in, inv_n, scratch, Mx, My);
 
     double accC = 0.0, accS = 0.0;
     if (tid >= CONSUMERS) {
@@ -425,13 +426,29 @@ hmf_cluster_kernel(double* __restrict__ theta, double* __restrict__ p, long long
     if (rank == 0 && tid < C) partial_out[tid] = cta_part[parity ^ 1][tid];
 }
 
+// Sharded runs ("each GPU computes its contribution to the magnetisation, which are then summed"):
+// the per-CTA partials of this rank, added in index order, as ONE (sum cos, sum sin) pair that the caller's
+// all-reduce sums over ranks in place; the next kernel then reads it with g_in = 1.
+__global__ void __launch_bounds__(kHmfThreads)
+hmf_collapse_kernel(const double2* __restrict__ partial_in, int g_in, double2* __restrict__ out1) {
+    __shared__ double scratch[2 * (kHmfThreads / 32)];
+    double v[2] = {0.0, 0.0};
+    for (int i = threadIdx.x; i < g_in; i += kHmfThreads) {
+        const double2 q = partial_in[i];
+        v[0] += q.x;
+        v[1] += q.y;
+    }
+    block_sum<kHmfThreads, 2>(v, scratch);
+    if (threadIdx.x == 0) *out1 = make_double2(v[0], v[1]);
+}
+
 // f_i = cos(theta_i) My - sin(theta_i) Mx  -> f   (lrmd_forces; eq.(6))
 __global__ void __launch_bounds__(kHmfThreads)
-hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long long N,
+hmf_force_kernel(const double* __restrict__ theta, double* __restrict__ f, long long N, double inv_n,
                  const double2* __restrict__ partial_in, int g_in) {
     __shared__ double scratch[2 * (kHmfThreads / 32)];
     double Mx, My;
-    hmf_magnetisation<kHmfThreads>(partial_in, g_in, 1.0 / (double)N, scratch, Mx, My);
+    hmf_magnetisation<kHmfThreads>(partial_in, g_in, inv_n, scratch, Mx, My);
     const long long stride = (long long)gridDim.x * kHmfThreads;
     for (long long i = (long long)blockIdx.x * kHmfThreads + threadIdx.x; i < N; i += stride) {
         double s, c;
@@ -488,7 +505,7 @@ energy_finalize_kernel(int model, long long N, const double* __restrict__ kpart,
     double V, a = r[1], b = r[2];
     if (model == 0) {
         double Mx, My;
-        hmf_magnetisation<kHmfThreads>(mpart, g_m, 1.0 / (double)N, scratch, Mx, My);
+        hmf_magnetisation<kHmfThreads>(mpart, g_m, 1.0 / (double)N, scratch, Mx, My);   // N = all particles
         V = 0.5 * (double)N * (1.0 - Mx * Mx - My * My);
         a = Mx;
         b = My;

@@ -35,6 +35,7 @@ struct Layout {
     size_t partial1 = 0;      // [slots][N] (GRAV2D)
     size_t kpart = 0;         // 3 * kEnergyGrid
     size_t vpart = 0;         // one per CTA of the pair-energy kernel
+    size_t shared2 = 0;       // HMF shard: this rank's (sum cos, sum sin), all-reduced in place
     size_t total = 0;
 };
 
@@ -42,8 +43,13 @@ struct Layout {
 
 struct lrmd_ctx {
     int model = 0;
-    int64_t N = 0;
+    int64_t N = 0;              // particles this context owns (all of them unless it is a shard)
     double eps = 0.0;
+    // sharding (lrmd_set_shard): this context owns the global indices i0 .. i0 + N - 1 of N_total particles
+    int64_t N_total = 0, i0 = 0;
+    lrmd_allreduce_fn allreduce = nullptr;
+    lrmd_allgather_fn allgather = nullptr;
+    void* coll_user = nullptr;
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
     int64_t opt_hmf_variant = -1, opt_pair_variant = -1;
@@ -109,9 +115,10 @@ void resolve(lrmd_ctx* c) {
     Layout L;
     size_t off = 0;
     if (c->model == LRMD_HMF) {
+        const bool sharded = c->N_total != c->N;
         c->hmf_variant = c->opt_hmf_variant >= 0 ? (int)c->opt_hmf_variant
                          : (N >= kHmfTmaMinN ? 1 : (N <= kHmfClusterMaxN ? kHmfClusterVariant : 0));
-        if (c->hmf_variant == kHmfClusterVariant && N > kHmfClusterMaxN) c->hmf_variant = 0;
+        if (c->hmf_variant == kHmfClusterVariant && (N > kHmfClusterMaxN || sharded)) c->hmf_variant = 0;
         const HmfVariant hv = kHmfVariants[c->hmf_variant];
         int64_t g;
         if (c->hmf_variant == kHmfClusterVariant) {
@@ -132,13 +139,15 @@ void resolve(lrmd_ctx* c) {
         c->slots = 1;
         L.hmf_partial = off; off = align_up(off + 3 * sizeof(double2) * kHmfMaxGrid);
         c->use_graph = c->opt_graph < 0 ? (N <= (1 << 20)) : (c->opt_graph != 0);
-        if (c->hmf_variant == kHmfClusterVariant) c->use_graph = false;
+        if (c->hmf_variant == kHmfClusterVariant || sharded) c->use_graph = false;   // collectives between substages
+        L.shared2 = off; off = align_up(off + sizeof(double2));
     } else {
         c->pair_variant = c->opt_pair_variant >= 0 ? (int)c->opt_pair_variant : (c->model == LRMD_GRAV2D ? 1 : 0);
         int itile = 0, minb = 0;
         with_pair_cfg(c->pair_variant, [&](auto cfg) { itile = decltype(cfg)::ITILE; minb = decltype(cfg)::MINB; });
         const int64_t itiles = (N + itile - 1) / itile;
-        const int64_t Lpos = itiles * N;                       // flattened (i-tile, j) positions
+        const int64_t NJ = c->N_total;                         // j runs over all particles, also in a shard
+        const int64_t Lpos = itiles * NJ;                      // flattened (i-tile, j) positions
         const int64_t slots_hw = (int64_t)kNumSm * minb;       // resident CTAs on the device
         int64_t G;
         if (c->opt_pair_ctas > 0) {
@@ -146,7 +155,7 @@ void resolve(lrmd_ctx* c) {
         } else {
             // one wave of equal ranges for small N; for large N ranges of about max(64Ki, N/8) positions
             // (whole waves), which bounds both the tail of the last wave and the partial rows per tile
-            int64_t qt = N / 8 > 65536 ? N / 8 : 65536;
+            int64_t qt = NJ / 8 > 65536 ? NJ / 8 : 65536;
             int64_t waves = (Lpos + slots_hw * qt / 2) / (slots_hw * qt);
             if (waves < 1) waves = 1;
             G = slots_hw * waves;
@@ -156,7 +165,7 @@ void resolve(lrmd_ctx* c) {
         if (G > Lpos) G = Lpos;
         if (G < 1) G = 1;
         PairPart P;
-        P.N = N; P.G = (int)G; P.q = Lpos / G; P.r = Lpos % G; P.itile = itile;
+        P.N = NJ; P.Ni = N; P.i0 = c->i0; P.G = (int)G; P.q = Lpos / G; P.r = Lpos % G; P.itile = itile;
         c->part = P;
         int64_t smax = 1;
         for (int64_t t = 0; t < itiles; ++t) {
@@ -166,8 +175,8 @@ void resolve(lrmd_ctx* c) {
         }
         c->slots = (int)smax;
         c->hmf_grid = 0;
-        L.js = off; off = align_up(off + sizeof(double2) * (size_t)N);
-        if (c->opt_precision == 1) { L.js32 = off; off = align_up(off + sizeof(float2) * ((size_t)N + 2)); }
+        L.js = off; off = align_up(off + sizeof(double2) * (size_t)NJ);
+        if (c->opt_precision == 1) { L.js32 = off; off = align_up(off + sizeof(float2) * ((size_t)NJ + 2)); }
         L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots);
         if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots); }
         L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
@@ -268,6 +277,11 @@ struct Launcher {
 inline double2* hmf_buf(lrmd_ctx* c, int k) {
     return reinterpret_cast<double2*>(c->ws + c->lay.hmf_partial) + (size_t)k * kHmfMaxGrid;
 }
+inline bool is_sharded(const lrmd_ctx* c) { return c->N_total != c->N; }
+inline double2* shared2_ptr(lrmd_ctx* c) { return reinterpret_cast<double2*>(c->ws + c->lay.shared2); }
+// where the kernels read (sum cos, sum sin) from: the rank-summed pair of a shard, or the per-CTA partials
+inline const double2* hmf_sums(lrmd_ctx* c, int buf) { return is_sharded(c) ? shared2_ptr(c) : hmf_buf(c, buf); }
+inline int hmf_nsums(const lrmd_ctx* c) { return is_sharded(c) ? 1 : c->hmf_grid; }
 inline double2* js_ptr(lrmd_ctx* c) { return reinterpret_cast<double2*>(c->ws + c->lay.js); }
 inline float2* js32_ptr(lrmd_ctx* c) {
     return c->opt_precision == 1 ? reinterpret_cast<float2*>(c->ws + c->lay.js32) : nullptr;
@@ -294,12 +308,14 @@ template <bool KICK, bool KICK2, bool DRIFT, bool REDUCE>
 void hmf_launch(Launcher& L, bool timed, double kickA, double kickB, double drift, int in_buf, int out_buf) {
     lrmd_ctx* c = L.c;
     const dim3 g(c->hmf_grid);
-    const double2* pin = hmf_buf(c, in_buf);
+    const double2* pin = hmf_sums(c, in_buf);
+    const int gin = hmf_nsums(c);
+    const double inv_n = 1.0 / (double)c->N_total;
     double2* pout = hmf_buf(c, out_buf);
 #define LRMD_HMF_GO(KERNEL, BLOCK)                                                                           \
     do {                                                                                                     \
-        if (timed) L.go_timed(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, kickA, kickB, drift, pin, c->hmf_grid, pout); \
-        else L.go(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, kickA, kickB, drift, pin, c->hmf_grid, pout);     \
+        if (timed) L.go_timed(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, inv_n, kickA, kickB, drift, pin, gin, pout); \
+        else L.go(KERNEL, g, dim3(BLOCK), c->a0, c->a1, c->N, inv_n, kickA, kickB, drift, pin, gin, pout);     \
     } while (0)
 #define LRMD_HMF_TMA(V, CONS, NS, MINB)                                                                      \
     case V:                                                                                                  \
@@ -315,6 +331,11 @@ void hmf_launch(Launcher& L, bool timed, double kickA, double kickB, double drif
     }
 #undef LRMD_HMF_TMA
 #undef LRMD_HMF_GO
+    if (REDUCE && is_sharded(c)) {
+        // each GPU's contribution to the magnetisation, summed over the GPUs
+        L.go(hmf_collapse_kernel, dim3(1), dim3(kHmfThreads), (const double2*)pout, c->hmf_grid, shared2_ptr(c));
+        if (L.rc == LRMD_OK && c->allreduce && c->allreduce(shared2_ptr(c), 2, L.stream, c->coll_user) != 0) L.rc = LRMD_ECOLL;
+    }
 }
 
 // One fused substage: [kick kickA (+kickB)] -> drift -> reduce into the next partial buffer.
@@ -440,11 +461,24 @@ int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
 
 // ---- pair-model sequencing ---------------------------------------------------------------------------
 
+// Shards: every rank needs all positions for its rows' pair sums ("each GPU holds all
+// positions"; the paper copies halves peer to peer, here the caller's all-gather fills the packed stream in place).
+void pair_gather(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    if (!is_sharded(c) || !c->allgather || L.rc != LRMD_OK) return;
+    if (c->allgather(js_ptr(c), (int64_t)sizeof(double2), c->i0, c->N, c->N_total, L.stream, c->coll_user) != 0) L.rc = LRMD_ECOLL;
+    if (L.rc == LRMD_OK && js32_ptr(c) &&
+        c->allgather(js32_ptr(c), (int64_t)sizeof(float2), c->i0, c->N, c->N_total, L.stream, c->coll_user) != 0)
+        L.rc = LRMD_ECOLL;
+}
+
 void pair_pack(Launcher& L) {
     lrmd_ctx* c = L.c;
     const dim3 g((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), b(kUpdThreads);
-    if (c->model == LRMD_RING) L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, js_ptr(c), (float2*)nullptr);
-    else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, js_ptr(c), js32_ptr(c));
+    if (c->model == LRMD_RING)
+        L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, c->i0, js_ptr(c), (float2*)nullptr);
+    else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, c->i0, js_ptr(c), js32_ptr(c));
+    pair_gather(L);
 }
 
 void pair_force(Launcher& L) {
@@ -454,12 +488,12 @@ void pair_force(Launcher& L) {
         const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
         if (c->model == LRMD_RING)
             L.go_timed(pair_force_kernel<1, CFG>, g, b, js_ptr(c), c->part, c->eps,
-                       -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N), part0(c), part1(c));
+                       -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N_total), part0(c), part1(c));
         else if (c->opt_precision == 1)
             L.go_timed(grav_force_f32_kernel<CFG>, g, b, (const float2*)js32_ptr(c), c->part, (float)c->eps,
-                       -2.0 / (double)c->N, part0(c), part1(c));
+                       -2.0 / (double)c->N_total, part0(c), part1(c));
         else
-            L.go_timed(pair_force_kernel<2, CFG>, g, b, js_ptr(c), c->part, c->eps, -2.0 / (double)c->N, part0(c),
+            L.go_timed(pair_force_kernel<2, CFG>, g, b, js_ptr(c), c->part, c->eps, -2.0 / (double)c->N_total, part0(c),
                        part1(c));
     });
 }
@@ -481,6 +515,7 @@ void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB
         else LRMD_UPD(2, false, true);
     }
 #undef LRMD_UPD
+    if (drift) pair_gather(L);   // the packed stream changed: every rank needs the new positions
 }
 
 void pair_ensure_force(Launcher& L) {
@@ -524,6 +559,7 @@ int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps) {
     if (!c) return LRMD_EINVAL;
     c->model = model;
     c->N = N;
+    c->N_total = N;
     c->eps = (model == LRMD_HMF) ? 0.0 : eps;
     resolve(c);
     *out = c;
@@ -627,7 +663,7 @@ int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
         int64_t g = (c->N + kHmfThreads - 1) / kHmfThreads;
         if (g > kHmfMaxGrid) g = kHmfMaxGrid;
         L.go(hmf_force_kernel, dim3((unsigned)g), dim3(kHmfThreads), (const double*)c->a0, f0, c->N,
-             (const double2*)hmf_buf(c, c->cur), c->hmf_grid);
+             1.0 / (double)c->N_total, hmf_sums(c, c->cur), hmf_nsums(c));
     } else {
         pair_ensure_force(L);
         L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->part,
@@ -649,8 +685,8 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
     L.go(kinetic_partial_kernel, dim3((unsigned)gk), dim3(kHmfThreads), p0, p1, c->N, kpart(c));
     if (c->model == LRMD_HMF) {
         if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }
-        L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
-             (const double2*)hmf_buf(c, c->cur), c->hmf_grid, (const double*)nullptr, 0, out4_device);
+        L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N_total, (const double*)kpart(c), (int)gk,
+             hmf_sums(c, c->cur), hmf_nsums(c), (const double*)nullptr, 0, out4_device);
     } else {
         if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
         // V = pre * sum_{i<j} t_ij = (pre/2) * sum_{i != j} t_ij
@@ -659,15 +695,36 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
             const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
             if (c->model == LRMD_RING)
                 L.go(pair_energy_kernel<1, CFG>, g, b, (const double2*)js_ptr(c), c->part, c->eps,
-                     -0.5 / (std::sqrt(2.0) * (double)c->N), vpart(c));
+                     -0.5 / (std::sqrt(2.0) * (double)c->N_total), vpart(c));
             else
-                L.go(pair_energy_kernel<2, CFG>, g, b, (const double2*)js_ptr(c), c->part, c->eps, 0.5 / (double)c->N,
+                L.go(pair_energy_kernel<2, CFG>, g, b, (const double2*)js_ptr(c), c->part, c->eps, 0.5 / (double)c->N_total,
                      vpart(c));
         });
         L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
              (const double2*)nullptr, 0, (const double*)vpart(c), c->part.G, out4_device);
     }
     return L.rc;
+}
+
+int lrmd_set_shard(lrmd_ctx* c, int64_t N_total, int64_t i0, lrmd_allreduce_fn allreduce, lrmd_allgather_fn allgather,
+                   void* user) {
+    if (!c) return LRMD_EINVAL;
+    if (i0 < 0 || N_total < c->N || i0 + c->N > N_total) return LRMD_EINVAL;
+    if (c->model != LRMD_HMF && N_total > ((int64_t)1 << 28)) return LRMD_EINVAL;
+    const bool shard = N_total != c->N;
+    if (shard && (c->model == LRMD_HMF ? !allreduce : !allgather)) return LRMD_EINVAL;
+    c->N_total = N_total;
+    c->i0 = i0;
+    c->allreduce = allreduce;
+    c->allgather = allgather;
+    c->coll_user = user;
+    const size_t before = c->lay.total;
+    resolve(c);
+    drop_graph(c);
+    c->force_valid = false;
+    c->js_valid = false;
+    if (c->lay.total > before) c->ws = nullptr;   // back to "workspace not set"
+    return LRMD_OK;
 }
 
 int lrmd_step_observe(lrmd_ctx* c, int64_t n, double dt, int64_t every, double* out_device, void* cuda_stream) {
@@ -783,6 +840,7 @@ const char* lrmd_strerror(int code) {
         case LRMD_ESTATE: return "state or workspace not set";
         case LRMD_ECUDA: return "CUDA error (see lrmd_last_cuda_error)";
         case LRMD_EUNSUPPORTED: return "not implemented in this build";
+        case LRMD_ECOLL: return "a collective callback of a sharded context failed";
         default: return "unknown error code";
     }
 }

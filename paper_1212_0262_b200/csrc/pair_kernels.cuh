@@ -46,7 +46,9 @@ struct PairCfg {
 // force row partial[slot][i], slot = cta - (first CTA touching the tile), and the update kernel
 // adds a tile's slots in slot order: deterministic, no atomics.
 struct PairPart {
-    long long N;      // particles
+    long long N;      // particles = j-elements of the packed stream (all of them, on every rank)
+    long long Ni;     // rows (i-particles) this context owns: global indices i0 .. i0 + Ni - 1
+    long long i0;     //   (Ni = N, i0 = 0 unless the context is one shard of a multi-GPU run)
     long long q, r;   // range lengths: q + 1 for CTAs < r, q for the others (q >= 1)
     int G;            // CTAs
     int itile;        // rows per i-tile
@@ -198,7 +200,7 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
     __shared__ PairSmem<double2, TJ> sm;
     JTilePipe<double2, TJ> pipe(sm);
     pipe.init();
-    const long long N = P.N;
+    const long long N = P.Ni;     // rows of this context; partial rows have this stride
     const double onepe = 1.0 + eps;
 
     PairSegments segs(P, blockIdx.x);
@@ -210,7 +212,7 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long i = ibase + (long long)r * THREADS;
-            const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
+            const double2 q = (i < N) ? js[P.i0 + i] : make_double2(0.0, 0.0);
             a[r] = q.x;
             b[r] = q.y;
             f0[r] = 0.0;
@@ -256,7 +258,7 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
             const long long i = ibase + (long long)r * THREADS;
             if (i < N) {
                 if (MODEL == 1) {
-                    if (i >= jbeg && i < jend) {   // remove the rounding-level j = i term again
+                    if (P.i0 + i >= jbeg && P.i0 + i < jend) {   // remove the rounding-level j = i term again
                         double c, p;
                         ring_pair_parts(a[r], b[r], make_double2(a[r], b[r]), onepe, c, p);
                         f0[r] -= __dmul_rn(c, p);   // the rounded product, so that N = 1 gives exactly 0
@@ -295,7 +297,7 @@ grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, do
     __shared__ PairSmem<float2, TJ> sm;
     JTilePipe<float2, TJ> pipe(sm);
     pipe.init();
-    const long long N = P.N;
+    const long long N = P.Ni;
 
     PairSegments segs(P, blockIdx.x);
     long long tile, jbeg, jend;
@@ -307,7 +309,7 @@ grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, do
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long i = ibase + (long long)r * THREADS;
-            const float2 q = (i < N) ? js32[i] : make_float2(0.f, 0.f);
+            const float2 q = (i < N) ? js32[P.i0 + i] : make_float2(0.f, 0.f);
             a[r] = q.x;
             b[r] = q.y;
             f0[r] = 0.0;
@@ -371,7 +373,7 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
     __shared__ double scratch[THREADS / 32];
     JTilePipe<double2, TJ> pipe(sm);
     pipe.init();
-    const long long N = P.N;
+    const long long N = P.Ni;
     const double onepe = 1.0 + eps;
     constexpr double kLn2 = 0x1.62e42fefa39efp-1;
     double vsum = 0.0;
@@ -386,8 +388,8 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long i = ibase + (long long)r * THREADS;
-            irow[r] = i;
-            const double2 q = (i < N) ? js[i] : make_double2(0.0, 0.0);
+            irow[r] = (i < N) ? P.i0 + i : -1;      // global index of the row, -1 for padding rows
+            const double2 q = (i < N) ? js[P.i0 + i] : make_double2(0.0, 0.0);
             a[r] = q.x;
             b[r] = q.y;
             acc[r] = 0.0;
@@ -396,13 +398,13 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
         pipe.run(js, jbeg, jend, [&](const double2* tl, int cnt, long long j0) {
             // only j-tiles that meet this i-tile's own rows can hold a j = i pair: they take the
             // masked sweep, all others the plain one (no compare / select per pair)
-            const long long ilo = tile * CFG::ITILE;
+            const long long ilo = P.i0 + tile * CFG::ITILE;
             const bool diag = (j0 < ilo + CFG::ITILE) && (j0 + cnt > ilo);
             int jself[R];   // j - j0 of the row's own index (outside [0, cnt) if not in this tile)
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const long long dj = irow[r] - j0;
-                jself[r] = (dj >= 0 && dj < cnt) ? (int)dj : -1;
+                jself[r] = (irow[r] >= 0 && dj >= 0 && dj < cnt) ? (int)dj : -1;
             }
             auto sweep = [&](auto masked) {
                 constexpr bool MASK = decltype(masked)::value;
@@ -458,7 +460,7 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
         });
 #pragma unroll
         for (int r = 0; r < R; ++r)
-            if (irow[r] < N) vsum += acc[r];
+            if (irow[r] >= 0) vsum += acc[r];
     }
 
     double v[1] = {vsum};
@@ -473,17 +475,17 @@ constexpr int kUpdThreads = 256;
 // js[i] = (cos th_i, sin th_i) (Ring; "computed and stored in global memory") or (x_i, y_i) (2D)
 template <int MODEL>
 __global__ void __launch_bounds__(kUpdThreads)
-pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, long long N, double2* __restrict__ js,
-                 float2* __restrict__ js32) {
+pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, long long N, long long i0,
+                 double2* __restrict__ js, float2* __restrict__ js32) {
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
     if (MODEL == 1) {
         double s, c;
         sincos_any(q0[i], s, c);
-        js[i] = make_double2(c, s);
+        js[i0 + i] = make_double2(c, s);
     } else {
-        js[i] = make_double2(q0[i], q1[i]);
-        if (js32) js32[i] = make_float2((float)q0[i], (float)q1[i]);
+        js[i0 + i] = make_double2(q0[i], q1[i]);
+        if (js32) js32[i0 + i] = make_float2((float)q0[i], (float)q1[i]);
     }
 }
 
@@ -501,7 +503,7 @@ __global__ void __launch_bounds__(kUpdThreads)
 pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __restrict__ p0, double* __restrict__ p1,
                    PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
                    double kickA, double kickB, double drift, double2* __restrict__ js, float2* __restrict__ js32) {
-    const long long N = P.N;
+    const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
     const int S = tile_slots(P, i);
@@ -524,12 +526,12 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
         if (MODEL == 2) {
             const double y = fma(drift, pb, q1[i]);
             q1[i] = y;
-            js[i] = make_double2(x, y);
-            if (js32) js32[i] = make_float2((float)x, (float)y);
+            js[P.i0 + i] = make_double2(x, y);
+            if (js32) js32[P.i0 + i] = make_float2((float)x, (float)y);
         } else {
             double sn, cs;
             sincos_any(x, sn, cs);
-            js[i] = make_double2(cs, sn);
+            js[P.i0 + i] = make_double2(cs, sn);
         }
     }
 }
@@ -538,7 +540,7 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
 __global__ void __launch_bounds__(kUpdThreads)
 pair_force_out_kernel(PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
                       double* __restrict__ f0, double* __restrict__ f1) {
-    const long long N = P.N;
+    const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
     const int S = tile_slots(P, i);

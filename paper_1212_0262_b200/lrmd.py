@@ -16,7 +16,7 @@ import ctypes as C
 import os
 
 HMF, RING, GRAV2D = 0, 1, 2
-OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED, ECOLL = 0, -1, -2, -3, -4, -5
 OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
 OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS = 5, 6, 7
 
@@ -25,7 +25,7 @@ SYMBOLS = (
     "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
-    "lrmd_pair_partition", "lrmd_step_observe",
+    "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard",
 )
 
 _lib = None
@@ -77,6 +77,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_host_sincos.argtypes = [_vp, _i64, _vp, _vp]
     lib.lrmd_pair_partition.argtypes = [_vp, _i64, _vp, _i64, C.POINTER(_i64)]
     lib.lrmd_step_observe.argtypes = [_vp, _i64, _dbl, _i64, _vp, _vp]
+    lib.lrmd_set_shard.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int

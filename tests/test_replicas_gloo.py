@@ -72,3 +72,61 @@ def test_reference_arm_line_rank0(workload):
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "particle-steps/s"
+
+
+# ---- sharding plumbing: bounds and the two collectives, gloo world 2 on CPU -------------
+
+def test_shard_bounds_cover_every_particle_once():
+    sys.path.insert(0, ROOT)
+    from paper_1212_0262_b200.sharded import shard_bounds
+    for n, w in ((10, 2), (10, 3), (7, 7), (1_048_576, 8), (50_000_000, 8), (5, 2)):
+        b = shard_bounds(n, w)
+        assert b[0][0] == 0 and sum(k for _, k in b) == n
+        for (i0, k), (j0, _) in zip(b[:-1], b[1:]):
+            assert i0 + k == j0
+        assert max(k for _, k in b) - min(k for _, k in b) <= 1
+
+
+def _coll_worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    from paper_1212_0262_b200.sharded import TorchDistCollectives, shard_bounds
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    coll = TorchDistCollectives(dist, rank, world)
+    # HMF exchange: each rank's (sum cos, sum sin), summed in place
+    t = torch.tensor([1.0 + rank, 10.0 * (rank + 1)], dtype=torch.float64)
+    coll.all_reduce_sum_(t)
+    res = {"sum": t.tolist()}
+    # pair-model exchange: packed 16-byte elements, equal shards (n = 6) and unequal shards (n = 7)
+    for n in (6, 7):
+        bounds = shard_bounds(n, world)
+        whole = torch.zeros(n * 16, dtype=torch.uint8)
+        i0, k = bounds[rank]
+        whole[i0 * 16:(i0 + k) * 16] = rank + 1
+        coll.all_gather_inplace_(whole, [(b * 16, (b + m) * 16) for b, m in bounds])
+        res[f"gather{n}"] = whole.view(-1, 16)[:, 0].tolist()
+    out[rank] = res
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharding_collectives_gloo_world2():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    with ctx.Manager() as m:
+        out = m.dict()
+        port = 29500 + (os.getpid() + 7) % 1000
+        procs = [ctx.Process(target=_coll_worker, args=(r, 2, port, out)) for r in range(2)]
+        for p in procs:
+            p.start()
+        for p in procs:
+            p.join(120)
+            assert p.exitcode == 0
+        res = dict(out)
+    for r in (0, 1):
+        assert res[r]["sum"] == [3.0, 30.0]
+        assert res[r]["gather6"] == [1, 1, 1, 2, 2, 2]
+        assert res[r]["gather7"] == [1, 1, 1, 2, 2, 2, 2]
