@@ -42,6 +42,10 @@ FP64_LANES_PER_SM = 64          # DFMA lanes per SM (guide: 148 SMs; FP64 issue 
 # flops per ordered pair with FMA = 2: Ring 7 DFMA + 4 DMUL = 18; 2D 7 DFMA + 2 DADD = 16
 PAIR_FLOP = {1: 18.0, 2: 16.0}
 PAIR_FP64_INSTR = {1: 11.0, 2: 9.0}
+# symmetric kernel (row N4): per UNORDERED pair Ring 8 DFMA + 4 DMUL, 2D 9 DFMA + 2 DADD = 20 flop; the figures below are
+# per ordered pair delivered (half), i.e. the work the kernel EXECUTES, not the ordered-pair convention
+SYM_PAIR_FLOP = {1: 10.0, 2: 10.0}
+SYM_PAIR_FP64_INSTR = {1: 6.0, 2: 5.5}
 HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
@@ -144,7 +148,7 @@ def units_per_force(w):
     return "pair-interactions/s", "pair-interactions/s", float(w.N) * float(w.N)
 
 
-def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False):
+def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False, ordered_pairs=False):
     import torch
     from paper_1212_0262_b200 import lrmd
 
@@ -152,7 +156,8 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     peaks = measured_peaks()
     st = w.state()
     ctx = lrmd.Context(w.model, w.N, w.eps, device=dev,
-                       options=({lrmd.OPT_PAIR_PRECISION: 1} if f32_pairs else None))
+                       options=({lrmd.OPT_PAIR_PRECISION: 1} if f32_pairs else
+                                ({lrmd.OPT_PAIR_SYMMETRIC: 0} if (ordered_pairs and w.model != 0) else None)))
     ctx.set_state(*st)
     stream = torch.cuda.current_stream(dev)
     state_bytes = ctx.narrays * w.N * 8
@@ -215,7 +220,8 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         "options": {"pair_ctas": ctx.get_option(lrmd.OPT_PAIR_CTAS), "pair_variant": ctx.get_option(lrmd.OPT_PAIR_VARIANT),
                     "pair_slots": ctx.get_option(lrmd.OPT_PAIR_SLOTS), "graph": ctx.get_option(lrmd.OPT_GRAPH),
                     "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT),
-                    "pair_precision": ctx.get_option(lrmd.OPT_PAIR_PRECISION)},
+                    "pair_precision": ctx.get_option(lrmd.OPT_PAIR_PRECISION),
+                    "pair_symmetric": ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC)},
     }
 
     # ---- roofline of the dominant kernel: second pass with an event pair around each of its launches
@@ -248,19 +254,28 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                     "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: 6 FADD/FFMA per pair",
                     "algorithmic_mufu_per_launch": mufu}
         else:
-            flop = PAIR_FLOP[w.model] * w.N * w.N
+            sym = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
+            flop = (SYM_PAIR_FLOP if sym else PAIR_FLOP)[w.model] * w.N * w.N
             achieved = flop / avg_s / 1e12
             peak = SM_COUNT * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-            instr_rate = PAIR_FP64_INSTR[w.model] * w.N * w.N / avg_s
+            instr_rate = (SYM_PAIR_FP64_INSTR if sym else PAIR_FP64_INSTR)[w.model] * w.N * w.N / avg_s
             roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                     "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",
                     "algorithmic_flop_per_launch": flop,
                     "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
                     "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
-        roof.update({"kernel": ("hmf_cluster_kernel" if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3 else "hmf_substage_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else "pair_force_kernel"),
+            if sym:
+                roof["note"] = ("symmetric kernel: every unordered pair evaluated once (N^2/2 evaluations deliver N^2 pair "
+                                "interactions); flops and instructions are the EXECUTED ones; by the ordered-pair convention "
+                                "(%g flop per delivered pair) the same launch reads %.3f of peak"
+                                % (PAIR_FLOP[w.model], PAIR_FLOP[w.model] * w.N * w.N / avg_s / 1e12 / peak))
+        roof.update({"kernel": ("hmf_cluster_kernel" if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3 else "hmf_substage_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else
+                                 ("pair_force_sym_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "pair_force_kernel")),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
-                     "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else ""))})
+                     "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else "") +
+                                                      ("_sym" if (w.model != 0 and not f32_pairs and
+                                                                  ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1) else ""))})
         out["roofline"] = roof
 
     # ---- energy sums (rows a-E1..a-E3), timed apart from the steps
@@ -435,6 +450,13 @@ def main():
             others[key] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options",
                                               "clocks", "roofline", "e2e", "energy") if k in r}
             others[key]["steps"] = DEFAULT_STEPS[key]
+        # the paper's own scheme, every ORDERED pair, on the configs where the symmetric kernel is the default
+        for key in ("ring_16k", "grav2d_64k"):
+            ow = inputs.WORKLOADS[key]
+            r = run_workload(ow, DEFAULT_STEPS[key], 3, None, with_e2e=False, ordered_pairs=True)
+            others[key + "_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
+                                                                 "options", "clocks", "roofline") if k in r}
+            others[key + "_ordered_pairs"]["steps"] = DEFAULT_STEPS[key]
         # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
         r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)
         others["grav2d_1m_f32pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",

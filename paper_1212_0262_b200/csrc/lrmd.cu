@@ -36,6 +36,7 @@ struct Layout {
     size_t kpart = 0;         // 3 * kEnergyGrid
     size_t vpart = 0;         // one per CTA of the pair-energy kernel
     size_t shared2 = 0;       // HMF shard: this rank's (sum cos, sum sin), all-reduced in place
+    size_t sym_wstart = 0, sym_tiles = 0, ipart0 = 0, ipart1 = 0, jpart0 = 0, jpart1 = 0;   // symmetric kernel
     size_t total = 0;
 };
 
@@ -52,11 +53,16 @@ struct lrmd_ctx {
     void* coll_user = nullptr;
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
-    int64_t opt_hmf_variant = -1, opt_pair_variant = -1;
+    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1;
     // resolved
     int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
     int slots = 1;              // partial force rows per particle (pair models)
     lrmd::PairPart part{};      // work partition of the pair kernels
+    bool sym = false;           // symmetric (Newton's third law) force kernel in use
+    lrmd::SymPart spart{};      // its work partition; the two tables below are uploaded by lrmd_set_workspace
+    std::vector<int4> sym_wstart;
+    std::vector<int2> sym_tiles;
+    int sym_slots = 1, sym_R = 4;
     bool use_graph = false;
     Layout lay;
     // bindings
@@ -108,6 +114,59 @@ void with_pair_cfg(int v, F f) {
         case 2: f(PairCfg2{}); break;
         default: f(PairCfg0{}); break;
     }
+}
+
+// Symmetric force kernel (row N4): decide whether it is used and build its work tables.
+// Units are (tile, chunk) pairs in tile-major order, chunk >= tile * R; G workers get equal contiguous shares.
+void resolve_sym(lrmd_ctx* c, int /*minb*/) {
+    c->sym = false;
+    c->sym_wstart.clear();
+    c->sym_tiles.clear();
+    const int64_t N = c->N;
+    if (c->opt_sym == 0 || c->N_total != c->N || c->opt_precision != 0) return;
+    const int R = c->pair_variant == 1 ? 8 : 4;
+    const int T = 32 * R;
+    const int64_t ntiles = (N + T - 1) / T, nchunks = (N + 31) / 32;
+    const int comps = c->model == LRMD_GRAV2D ? 2 : 1;
+    const double jbytes = (double)ntiles * (double)N * 8.0 * comps;
+    // the j-side rows cost ntiles x N doubles per component: automatic only up to 1 GiB, on request up to 64 GiB
+    if (jbytes > (c->opt_sym == 1 ? 64.0 : 1.0) * 1073741824.0) return;
+    if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
+    int64_t U = 0;
+    for (int64_t a = 0; a < ntiles; ++a) U += nchunks - a * R;
+    // workers: R = 4 (80 registers) keeps 24 warps per SM resident, R = 8 (138 registers) 12; measured best at
+    // 32 and 12 workers per SM (profiles/); at least two units per worker
+    int64_t G = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * (R == 8 ? 12 : 32);
+    if (c->opt_pair_ctas <= 0 && G > U / 2) G = U / 2;
+    if (G > U) G = U;
+    if (G < 1) G = 1;
+    c->sym_wstart.resize((size_t)G);
+    c->sym_tiles.assign((size_t)ntiles, make_int2(0x7fffffff, -1));
+    int64_t a = 0, cum = 0;     // cum = units before tile a
+    for (int64_t w = 0; w < G; ++w) {
+        const int64_t u0 = (w * U) / G, u1 = ((w + 1) * U) / G;
+        while (u0 >= cum + (nchunks - a * R)) { cum += nchunks - a * R; ++a; }
+        c->sym_wstart[(size_t)w] = make_int4((int)a, (int)(a * R + (u0 - cum)), (int)(u1 - u0), 0);
+        // tiles this worker touches
+        int64_t aa = a, cc = cum;
+        for (;;) {
+            int2& r = c->sym_tiles[(size_t)aa];
+            if ((int)w < r.x) r.x = (int)w;
+            if ((int)w > r.y) r.y = (int)w;
+            if (u1 <= cc + (nchunks - aa * R)) break;
+            cc += nchunks - aa * R;
+            ++aa;
+        }
+    }
+    int smax = 1;
+    for (const int2& r : c->sym_tiles) if (r.y - r.x + 1 > smax) smax = r.y - r.x + 1;
+    c->sym_slots = smax;
+    c->sym_R = R;
+    lrmd::SymPart S;
+    S.N = N; S.T = T; S.ntiles = (int)ntiles; S.nchunks = (int)nchunks; S.G = (int)G;
+    S.wstart = nullptr; S.tile_rng = nullptr;
+    c->spart = S;
+    c->sym = true;
 }
 
 void resolve(lrmd_ctx* c) {
@@ -175,10 +234,21 @@ void resolve(lrmd_ctx* c) {
         }
         c->slots = (int)smax;
         c->hmf_grid = 0;
+        resolve_sym(c, minb);
         L.js = off; off = align_up(off + sizeof(double2) * (size_t)NJ);
         if (c->opt_precision == 1) { L.js32 = off; off = align_up(off + sizeof(float2) * ((size_t)NJ + 2)); }
-        L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots);
-        if (c->model == LRMD_GRAV2D) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->slots); }
+        const bool two = c->model == LRMD_GRAV2D;
+        const size_t rows = c->sym ? 1 : (size_t)c->slots;     // symmetric: one folded row
+        L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * rows);
+        if (two) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * rows); }
+        if (c->sym) {
+            L.sym_wstart = off; off = align_up(off + sizeof(int4) * c->sym_wstart.size());
+            L.sym_tiles = off; off = align_up(off + sizeof(int2) * c->sym_tiles.size());
+            L.ipart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots);
+            if (two) { L.ipart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots); }
+            L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->spart.ntiles);
+            if (two) { L.jpart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->spart.ntiles); }
+        }
         L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
         c->use_graph = false;
     }
@@ -481,8 +551,29 @@ void pair_pack(Launcher& L) {
     pair_gather(L);
 }
 
+inline double* wsd(lrmd_ctx* c, size_t off) { return off ? reinterpret_cast<double*>(c->ws + off) : nullptr; }
+
+// Symmetric force evaluation (row N4) + the fold into one force row.
+void pair_force_sym(Launcher& L) {
+    lrmd_ctx* c = L.c;
+    const dim3 g((unsigned)((c->spart.G + kSymThreads / 32 - 1) / (kSymThreads / 32))), b(kSymThreads);
+    double *i0 = wsd(c, c->lay.ipart0), *i1 = wsd(c, c->lay.ipart1), *j0 = wsd(c, c->lay.jpart0), *j1 = wsd(c, c->lay.jpart1);
+    if (c->model == LRMD_RING) {
+        const double pre = -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N);
+        if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<1, 8>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
+        else L.go_timed(pair_force_sym_kernel<1, 4>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
+    } else {
+        const double pre = -2.0 / (double)c->N;
+        if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<2, 8>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
+        else L.go_timed(pair_force_sym_kernel<2, 4>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
+    }
+    L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N + 255) / 256)), dim3(256), c->spart, (const double*)i0,
+         (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
+}
+
 void pair_force(Launcher& L) {
     lrmd_ctx* c = L.c;
+    if (c->sym) { pair_force_sym(L); return; }
     with_pair_cfg(c->pair_variant, [&](auto cfg) {
         using CFG = decltype(cfg);
         const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
@@ -504,7 +595,7 @@ void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB
     double *q0 = c->a0, *q1 = nullptr, *p0 = c->a1, *p1 = nullptr;
     if (c->model == LRMD_GRAV2D) { q1 = c->a1; p0 = c->a2; p1 = c->a3; }
 #define LRMD_UPD(M, K2, DR) \
-    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, part0(c), part1(c), kickA, kickB, d, js_ptr(c), js32_ptr(c))
+    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, c->sym ? 1 : 0, part0(c), part1(c), kickA, kickB, d, js_ptr(c), js32_ptr(c))
     if (c->model == LRMD_RING) {
         if (!drift) LRMD_UPD(1, false, false);
         else if (kick2) LRMD_UPD(1, true, true);
@@ -581,10 +672,23 @@ int lrmd_workspace_bytes(const lrmd_ctx* c, size_t* bytes) {
 }
 
 int lrmd_set_workspace(lrmd_ctx* c, void* device_ptr, size_t bytes, void* cuda_stream) {
-    (void)cuda_stream;   // the workspace needs no initialisation: every buffer is written before it is read
+    // every buffer is written by a kernel before it is read, except the two small work tables of the symmetric
+    // pair kernel, which are copied here (host -> device on the given stream)
     if (!c || !device_ptr) return LRMD_EINVAL;
     if (bytes < c->lay.total || ((uintptr_t)device_ptr % kAlign) != 0) return LRMD_EINVAL;
     c->ws = static_cast<char*>(device_ptr);
+    if (c->sym) {
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        cudaError_t e = cudaMemcpyAsync(c->ws + c->lay.sym_wstart, c->sym_wstart.data(), sizeof(int4) * c->sym_wstart.size(),
+                                        cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(c->ws + c->lay.sym_tiles, c->sym_tiles.data(), sizeof(int2) * c->sym_tiles.size(),
+                                cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);    // the host vectors may change after this call
+        if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); c->ws = nullptr; return LRMD_ECUDA; }
+        c->spart.wstart = reinterpret_cast<const int4*>(c->ws + c->lay.sym_wstart);
+        c->spart.tile_rng = reinterpret_cast<const int2*>(c->ws + c->lay.sym_tiles);
+    }
     c->force_valid = false;
     c->js_valid = false;
     drop_graph(c);
@@ -667,7 +771,7 @@ int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
     } else {
         pair_ensure_force(L);
         L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->part,
-             (const double*)part0(c), (const double*)part1(c), f0, f1);
+             c->sym ? 1 : 0, (const double*)part0(c), (const double*)part1(c), f0, f1);
     }
     return L.rc;
 }
@@ -776,6 +880,11 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (c->model != LRMD_HMF && value != 0) return LRMD_EINVAL;
             c->opt_hmf_grid = value;
             break;
+        case LRMD_OPT_PAIR_SYMMETRIC:
+            if (value < -1 || value > 1) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
+            c->opt_sym = value;
+            break;
         case LRMD_OPT_KERNEL_TIMING:
             if (value != 0 && value != 1) return LRMD_EINVAL;
             c->timing = value != 0;
@@ -797,10 +906,11 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
     if (!c || !value) return LRMD_EINVAL;
     switch (key) {
         case LRMD_OPT_PAIR_PRECISION: *value = c->opt_precision; break;
-        case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : c->part.G; break;
+        case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : (c->sym ? c->spart.G : c->part.G); break;
         case LRMD_OPT_HMF_VARIANT: *value = c->hmf_variant; break;
         case LRMD_OPT_PAIR_VARIANT: *value = c->pair_variant; break;
-        case LRMD_OPT_PAIR_SLOTS: *value = c->slots; break;
+        case LRMD_OPT_PAIR_SLOTS: *value = c->sym ? c->sym_slots : c->slots; break;
+        case LRMD_OPT_PAIR_SYMMETRIC: *value = c->sym ? 1 : 0; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;

@@ -356,6 +356,189 @@ grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, do
     }
 }
 
+// ---- symmetric force kernels: Newton's third law ------------------------------------
+// The paper computes every ordered pair ("the symmetry ... would introduce unnecessary complications with no
+// significant speed gain").  On an FP64-issue-bound B200 kernel halving the pair evaluations is
+// the one large factor left: per UNORDERED pair 2D 7 + 2 + 2 = 11 and Ring 11 + 2 = 13 FP64 instructions, i.e.
+// 5.5 / 6.5 per ordered pair instead of 9 / 11.
+// Scheme (one warp = one worker, no shared memory, no barriers): a warp owns an i-tile of 32 x R particles in
+// registers (R per lane) and walks over chunks of 32 j-particles with index beyond its tile; lane l loads
+// j = 32 c + l, and the j-packet (position + the force it collects) travels once around the warp by
+// shuffles: in each of 32 steps every lane evaluates its R i-particles against the packet it holds, adds
+// +f to its own i-accumulators and -f to the packet.  After 32 steps the packet is home again carrying the
+// force of the whole i-tile on j: it is written to jpart[tile][j].  The chunks of the tile itself are walked
+// the same way but only the i-side is kept (each ordered pair of the tile is met once that way).
+// Work = (tile, chunk) units in tile-major order, divided evenly over the warps (table built on the host);
+// a warp's i-side sums go to ipart[slot][i] like the ordered kernel's, and pair_sym_fold_kernel adds a
+// particle's ipart rows and the jpart rows of all lower tiles in a fixed order: deterministic, no atomics.
+struct SymPart {
+    long long N;
+    int T;            // particles per i-tile = 32 R
+    int ntiles;       // ceil(N / T)
+    int nchunks;      // ceil(N / 32)
+    int G;            // workers (warps)
+    const int4* wstart;    // [G]  first unit of worker w: (tile, chunk, number of units, 0)
+    const int2* tile_rng;  // [ntiles] first and last worker touching the tile
+};
+
+constexpr int kSymThreads = 128;   // 4 independent workers per CTA
+
+template <int MODEL, int R, bool MASK, bool DIAG>
+__device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b)[R], const bool (&vi)[R],
+                                          double (&f0)[R], double (&f1)[R], double2 q, bool vq, double eps,
+                                          double onepe, double& g0, double& g1) {
+    const unsigned lane = threadIdx.x & 31u, src = (lane + 31u) & 31u;   // the packet moves to lane + 1
+#pragma unroll 4
+    for (int s = 0; s < 32; ++s) {
+        // the position part of the next packet is requested before this step's arithmetic; the force part
+        // is summed per step (h0, h1) and joins the travelling sum only at the end, so that the shuffle
+        // latency of g never sits on the pair arithmetic's dependency chain
+        const double qnx = __shfl_sync(0xffffffffu, q.x, src);
+        const double qny = __shfl_sync(0xffffffffu, q.y, src);
+        const bool vqn = MASK ? (__shfl_sync(0xffffffffu, (int)vq, src) != 0) : true;
+        double h0 = 0.0, h1 = 0.0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (MODEL == 2) {
+                const double dx = a[r] - q.x, dy = b[r] - q.y;
+                const double r2 = fma(dy, dy, fma(dx, dx, eps));
+                const double y0 = rcp_seed(r2);
+                const double e = fma(-r2, y0, 1.0);
+                const double t = fma(e, e, e);
+                double y = fma(y0, t, y0);
+                if (MASK) y = (vi[r] && vq) ? y : 0.0;
+                f0[r] = fma(dx, y, f0[r]);
+                f1[r] = fma(dy, y, f1[r]);
+                if (!DIAG) {
+                    h0 = fma(-dx, y, h0);
+                    h1 = fma(-dy, y, h1);
+                }
+            } else {
+                double c, p;
+                ring_pair_parts(a[r], b[r], q, onepe, c, p);
+                if (MASK) c = (vi[r] && vq) ? c : 0.0;
+                f0[r] = fma(c, p, f0[r]);
+                if (!DIAG) h0 = fma(-c, p, h0);
+            }
+        }
+        if (!DIAG) {
+            g0 = __shfl_sync(0xffffffffu, g0 + h0, src);
+            if (MODEL == 2) g1 = __shfl_sync(0xffffffffu, g1 + h1, src);
+        }
+        q.x = qnx;
+        q.y = qny;
+        if (MASK) vq = vqn;
+    }
+}
+
+template <int MODEL, int R>
+__global__ void __launch_bounds__(kSymThreads)
+pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, double pre, double* __restrict__ ipart0,
+                      double* __restrict__ ipart1, double* __restrict__ jpart0, double* __restrict__ jpart1) {
+    const int w = blockIdx.x * (kSymThreads / 32) + (threadIdx.x >> 5);
+    if (w >= S.G) return;
+    const int lane = threadIdx.x & 31;
+    const long long N = S.N;
+    const double onepe = 1.0 + eps;
+    const int4 st = S.wstart[w];
+    int tile = st.x, chunk = st.y;
+    const bool ragged = (N % S.T) != 0 || (N % 32) != 0;
+
+    double a[R], b[R], f0[R], f1[R];
+    bool vi[R];
+    unsigned selfmask = 0u;   // rows whose own chunk this worker walked since load_tile (Ring: self term to remove)
+    auto load_tile = [&](int t) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = (long long)t * S.T + r * 32 + lane;
+            vi[r] = i < N;
+            const double2 q = vi[r] ? js[i] : make_double2(0.0, 0.0);
+            a[r] = q.x;
+            b[r] = q.y;
+            f0[r] = 0.0;
+            f1[r] = 0.0;
+        }
+    };
+    auto store_tile = [&](int t) {
+        const int slot = w - S.tile_rng[t].x;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = (long long)t * S.T + r * 32 + lane;
+            if (MODEL == 1 && ((selfmask >> r) & 1u)) {
+                // remove the rounding-level j = i term of eq.(9) again (the rounded product: N = 1 gives exactly 0)
+                double c, p;
+                ring_pair_parts(a[r], b[r], make_double2(a[r], b[r]), onepe, c, p);
+                f0[r] -= __dmul_rn(c, p);
+            }
+            if (vi[r]) {
+                ipart0[(long long)slot * N + i] = pre * f0[r];
+                if (MODEL == 2) ipart1[(long long)slot * N + i] = pre * f1[r];
+            }
+        }
+    };
+    load_tile(tile);
+    long long jn = (long long)chunk * 32 + lane;
+    double2 qn = (jn < N) ? js[jn] : make_double2(0.0, 0.0);
+    for (int u = 0; u < st.z; ++u) {
+        const int ctile = tile, cchunk = chunk;
+        const long long j = jn;
+        const double2 q = qn;
+        const bool vq = j < N;
+        // the next unit, and its packet loaded before this unit's arithmetic
+        ++chunk;
+        const bool tile_done = chunk == S.nchunks;
+        if (tile_done) { ++tile; chunk = tile * R; }
+        const bool more = u + 1 < st.z;
+        if (more) {
+            jn = (long long)chunk * 32 + lane;
+            qn = (jn < N) ? js[jn] : make_double2(0.0, 0.0);
+        }
+        double g0 = 0.0, g1 = 0.0;
+        const bool diag = cchunk < (ctile + 1) * R;
+        const bool masked = ragged && (ctile == S.ntiles - 1 || cchunk == S.nchunks - 1);
+        if (diag) {
+            if (masked) sym_chunk<MODEL, R, true, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            else sym_chunk<MODEL, R, false, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            selfmask |= 1u << (cchunk - ctile * R);   // this walk met j = i for that row of every lane (step 0)
+        } else {
+            if (masked) sym_chunk<MODEL, R, true, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            else sym_chunk<MODEL, R, false, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            if (vq) {
+                jpart0[(long long)ctile * N + j] = pre * g0;
+                if (MODEL == 2) jpart1[(long long)ctile * N + j] = pre * g1;
+            }
+        }
+        if (tile_done || !more) {
+            store_tile(ctile);
+            if (more) load_tile(tile);
+        }
+    }
+}
+
+// f[i] = sum of the i-side rows of the workers that touched i's tile (slot order) + the j-side rows of all lower
+// tiles (tile order) -> out0 / out1 (row 0 of the partial force arrays).
+__global__ void __launch_bounds__(256)
+pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
+                     const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
+                     double* __restrict__ out1) {
+    const long long N = S.N;
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (i >= N) return;
+    const int t = (int)(i / S.T);
+    const int2 rng = S.tile_rng[t];
+    double f = 0.0, g = 0.0;
+    for (int s = 0; s <= rng.y - rng.x; ++s) {
+        f += ipart0[(long long)s * N + i];
+        if (ipart1) g += ipart1[(long long)s * N + i];
+    }
+    for (int a = 0; a < t; ++a) {
+        f += jpart0[(long long)a * N + i];
+        if (jpart1) g += jpart1[(long long)a * N + i];
+    }
+    out0[i] = f;
+    if (out1) out1[i] = g;
+}
+
 // ---- potential-energy kernels (rows a-E2, a-E3) ---------------------------------------------------------
 // Full N x N sweep with the same partition; the j = i term is masked out; CTA k writes
 // vpart[k] = pre_half * sum over its ranges of sum_{i in tile} sum_{j in range, j != i} t_ij
@@ -501,12 +684,12 @@ __device__ __forceinline__ int tile_slots(const PairPart& P, long long i) {
 template <int MODEL, bool KICK2, bool DRIFT>
 __global__ void __launch_bounds__(kUpdThreads)
 pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __restrict__ p0, double* __restrict__ p1,
-                   PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
+                   PairPart P, int fixed_slots, const double* __restrict__ partial0, const double* __restrict__ partial1,
                    double kickA, double kickB, double drift, double2* __restrict__ js, float2* __restrict__ js32) {
     const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
-    const int S = tile_slots(P, i);
+    const int S = fixed_slots > 0 ? fixed_slots : tile_slots(P, i);   // 1 after pair_sym_fold_kernel
     double f = partial0[i];
     for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
     double p = fma(kickA, f, p0[i]);
@@ -538,12 +721,12 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
 
 // lrmd_forces for the pair models: f = sum_s partial[s][i]
 __global__ void __launch_bounds__(kUpdThreads)
-pair_force_out_kernel(PairPart P, const double* __restrict__ partial0, const double* __restrict__ partial1,
-                      double* __restrict__ f0, double* __restrict__ f1) {
+pair_force_out_kernel(PairPart P, int fixed_slots, const double* __restrict__ partial0,
+                      const double* __restrict__ partial1, double* __restrict__ f0, double* __restrict__ f1) {
     const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
-    const int S = tile_slots(P, i);
+    const int S = fixed_slots > 0 ? fixed_slots : tile_slots(P, i);
     double f = partial0[i];
     for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
     f0[i] = f;

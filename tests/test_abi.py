@@ -69,6 +69,11 @@ def test_calls_before_state_and_workspace_are_estate(lrmd):
 
 def test_options(lrmd):
     rc, h = lrmd.lrmd_create(RING, 16384, 0.01)
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SYMMETRIC) == (lrmd.OK, 1)     # chosen for this size (row N4)
+    rc, W = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)
+    assert rc == lrmd.OK and W % 148 == 0                                        # workers (warps) of the symmetric kernel
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 2) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 0) == lrmd.OK        # the paper's every-ordered-pair scheme
     rc, G = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)
     assert rc == lrmd.OK and G % 148 == 0 and G >= 148   # whole waves of the 148 SMs
     rc, slots = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)
@@ -90,6 +95,7 @@ def test_options(lrmd):
     assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SLOTS)[1] in (6, 7)   # 6 equal ranges per tile, boundaries not tile-aligned
     lrmd.lrmd_destroy(h)
     rc, h = lrmd.lrmd_create(GRAV2D, 5000, 1e-3)
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 0) == lrmd.OK
     rc, b0 = lrmd.lrmd_workspace_bytes(h)
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.OK
     assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_PRECISION) == (lrmd.OK, 1)
@@ -114,6 +120,7 @@ def test_pair_partition_covers_every_pair_once(lrmd, model, N, G):
     pairs differs by at most one j-position, and slot numbers are 0..k-1 per tile with k <= PAIR_SLOTS."""
     rc, h = lrmd.lrmd_create(model, N, 1e-3)
     assert rc == lrmd.OK
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 0) == lrmd.OK    # the ordered kernels' partition
     if G:
         assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, G) == lrmd.OK
     ctas = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)[1]

@@ -406,6 +406,66 @@ def test_energy_any_partition(lrmd, ref, torch, S):
         assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1]
 
 
+# ---- symmetric (Newton's third law) force kernel ---------------------
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N", [1, 2, 3, 31, 32, 33, 127, 128, 129, 255, 257, 1000, 4099, 10_007])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_symmetric_force_kernel_matches_oracle(lrmd, ref, torch, model, N, variant):
+    """Every unordered pair once, +f / -f to both particles; i-tiles of 128 (variant 0) or 256 (variant 1) rows,
+    ragged last tile and last chunk, any number of workers."""
+    eps = _eps(model)
+    st = _state(model, N, 4000 + N)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    for workers in (0, 1, 5, 1000):
+        opts = {lrmd.OPT_PAIR_SYMMETRIC: 1, lrmd.OPT_PAIR_VARIANT: variant, lrmd.OPT_PAIR_CTAS: workers}
+        ctx = lrmd.Context(model, N, eps, options=opts)
+        assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
+        ctx.set_state(*st)
+        f = ctx.forces()
+        got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+        ctx.close()
+        _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+def test_symmetric_kernel_trajectory_momentum_and_reproducibility(lrmd, ref, torch, model):
+    eps = _eps(model)
+    N = 5001
+    st = _state(model, N, 88)
+    outs = []
+    for _ in range(2):
+        ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_SYMMETRIC: 1})
+        ctx.set_state(*st)
+        ctx.step(10, 0.01)
+        outs.append(ctx.state_numpy())
+        ctx.close()
+    for x, y in zip(*outs):
+        assert np.array_equal(x, y)
+    r = [a.copy() for a in st]
+    q0, q1 = _q(model, r)
+    p0, p1 = _p(model, r)
+    ref.step(model, eps, q0, q1, p0, p1, 10, 0.01, form=1)
+    for g, w in zip(outs[0], r):
+        assert np.max(np.abs(g - w)) <= XTOL
+    pk = (2, 3) if model == GRAV2D else (1,)
+    for k in pk:     # antisymmetric pair forces: total momentum conserved to rounding
+        assert abs(math.fsum(outs[0][k]) - math.fsum(st[k])) <= 1e-13 * math.fsum(np.abs(st[k]))
+
+
+def test_symmetric_default_choice(lrmd, torch):
+    a = lrmd.Context(RING, 16_384, 0.01)
+    b = lrmd.Context(GRAV2D, 65_536, 1e-3)
+    c = lrmd.Context(GRAV2D, 1_048_576, 1e-3)
+    d = lrmd.Context(GRAV2D, 65_536, 1e-3, options={lrmd.OPT_PAIR_SYMMETRIC: 0})
+    assert a.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and b.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
+    assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0      # 64 GiB of j-side rows: the ordered kernel stays
+    assert d.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0
+    for x in (a, b, c, d):
+        x.close()
+
+
 # ---- fp32 pair arithmetic (SURVEY.md 8(f) N1; PAPER.md:110) -----------------------------------------
 
 F32TOL = 1e-5    # north_star: 1e-5 * sum_j |f_ij| for the fp32 variant
