@@ -269,7 +269,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                                 "interactions); flops and instructions are the EXECUTED ones; by the ordered-pair convention "
                                 "(%g flop per delivered pair) the same launch reads %.3f of peak"
                                 % (PAIR_FLOP[w.model], PAIR_FLOP[w.model] * w.N * w.N / avg_s / 1e12 / peak))
-        roof.update({"kernel": ("hmf_cluster_kernel" if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3 else "hmf_substage_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else
+        roof.update({"kernel": {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else
                                  ("pair_force_sym_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "pair_force_kernel")),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,

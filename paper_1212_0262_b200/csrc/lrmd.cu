@@ -567,8 +567,17 @@ void pair_force_sym(Launcher& L) {
         if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<2, 8>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
         else L.go_timed(pair_force_sym_kernel<2, 4>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
     }
-    L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N + 255) / 256)), dim3(256), c->spart, (const double*)i0,
+    L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N + 31) / 32)), dim3(32, 8), c->spart, (const double*)i0,
          (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
+}
+
+
+ForceRows force_rows(lrmd_ctx* c) {
+    ForceRows FR;
+    FR.partial0 = part0(c);
+    FR.partial1 = part1(c);
+    FR.single_row = c->sym ? 1 : 0;
+    return FR;
 }
 
 void pair_force(Launcher& L) {
@@ -595,7 +604,7 @@ void pair_update(Launcher& L, bool kick2, bool drift, double kickA, double kickB
     double *q0 = c->a0, *q1 = nullptr, *p0 = c->a1, *p1 = nullptr;
     if (c->model == LRMD_GRAV2D) { q1 = c->a1; p0 = c->a2; p1 = c->a3; }
 #define LRMD_UPD(M, K2, DR) \
-    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, c->sym ? 1 : 0, part0(c), part1(c), kickA, kickB, d, js_ptr(c), js32_ptr(c))
+    L.go(pair_update_kernel<M, K2, DR>, g, b, q0, q1, p0, p1, c->part, force_rows(c), kickA, kickB, d, js_ptr(c), js32_ptr(c))
     if (c->model == LRMD_RING) {
         if (!drift) LRMD_UPD(1, false, false);
         else if (kick2) LRMD_UPD(1, true, true);
@@ -771,7 +780,7 @@ int lrmd_forces(lrmd_ctx* c, double* f0, double* f1, void* cuda_stream) {
     } else {
         pair_ensure_force(L);
         L.go(pair_force_out_kernel, dim3((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), dim3(kUpdThreads), c->part,
-             c->sym ? 1 : 0, (const double*)part0(c), (const double*)part1(c), f0, f1);
+             force_rows(c), f0, f1);
     }
     return L.rc;
 }

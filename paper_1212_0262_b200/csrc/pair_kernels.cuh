@@ -369,7 +369,7 @@ grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, do
 // force of the whole i-tile on j: it is written to jpart[tile][j].  The chunks of the tile itself are walked
 // the same way but only the i-side is kept (each ordered pair of the tile is met once that way).
 // Work = (tile, chunk) units in tile-major order, divided evenly over the warps (table built on the host);
-// a warp's i-side sums go to ipart[slot][i] like the ordered kernel's, and pair_sym_fold_kernel adds a
+// a warp's i-side sums go to ipart[slot][i] like the ordered kernel's, and the consumer adds a
 // particle's ipart rows and the jpart rows of all lower tiles in a fixed order: deterministic, no atomics.
 struct SymPart {
     long long N;
@@ -515,30 +515,6 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
     }
 }
 
-// f[i] = sum of the i-side rows of the workers that touched i's tile (slot order) + the j-side rows of all lower
-// tiles (tile order) -> out0 / out1 (row 0 of the partial force arrays).
-__global__ void __launch_bounds__(256)
-pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
-                     const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
-                     double* __restrict__ out1) {
-    const long long N = S.N;
-    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
-    if (i >= N) return;
-    const int t = (int)(i / S.T);
-    const int2 rng = S.tile_rng[t];
-    double f = 0.0, g = 0.0;
-    for (int s = 0; s <= rng.y - rng.x; ++s) {
-        f += ipart0[(long long)s * N + i];
-        if (ipart1) g += ipart1[(long long)s * N + i];
-    }
-    for (int a = 0; a < t; ++a) {
-        f += jpart0[(long long)a * N + i];
-        if (jpart1) g += jpart1[(long long)a * N + i];
-    }
-    out0[i] = f;
-    if (out1) out1[i] = g;
-}
-
 // ---- potential-energy kernels (rows a-E2, a-E3) ---------------------------------------------------------
 // Full N x N sweep with the same partition; the j = i term is masked out; CTA k writes
 // vpart[k] = pre_half * sum over its ranges of sum_{i in tile} sum_{j in range, j != i} t_ij
@@ -672,6 +648,49 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
     }
 }
 
+// Symmetric kernel's result for particle i: the i-side rows of the workers that touched i's tile + the j-side
+// rows of all lower tiles -> out0 / out1 (one force row).  Block = 32 particles x 8 row groups: group k adds
+// the rows k, k + 8, ... of each list in order, the 8 group sums are combined in a fixed tree: deterministic,
+// and eight times shorter than one dependent chain of ~100 loads per particle.
+__global__ void __launch_bounds__(256)
+pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
+                     const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
+                     double* __restrict__ out1) {
+    __shared__ double sf[8][32], sg[8][32];
+    const long long N = S.N;
+    const long long i = (long long)blockIdx.x * 32 + threadIdx.x;
+    const int k = threadIdx.y;
+    double f = 0.0, g = 0.0;
+    if (i < N) {
+        const int t = (int)(i / S.T);
+        const int2 rng = S.tile_rng[t];
+        for (int s = k; s <= rng.y - rng.x; s += 8) {
+            f += ipart0[(long long)s * N + i];
+            if (ipart1) g += ipart1[(long long)s * N + i];
+        }
+        for (int a = k; a < t; a += 8) {
+            f += jpart0[(long long)a * N + i];
+            if (jpart1) g += jpart1[(long long)a * N + i];
+        }
+    }
+    sf[k][threadIdx.x] = f;
+    sg[k][threadIdx.x] = g;
+    __syncthreads();
+    if (k == 0 && i < N) {
+        const int x = threadIdx.x;
+        out0[i] = ((sf[0][x] + sf[1][x]) + (sf[2][x] + sf[3][x])) + ((sf[4][x] + sf[5][x]) + (sf[6][x] + sf[7][x]));
+        if (out1) out1[i] = ((sg[0][x] + sg[1][x]) + (sg[2][x] + sg[3][x])) + ((sg[4][x] + sg[5][x]) + (sg[6][x] + sg[7][x]));
+    }
+}
+
+// The partial rows of a force evaluation: [slots][N] from the ordered kernels, or the single folded row of the
+// symmetric kernel (single_row = 1).
+struct ForceRows {
+    const double* partial0;
+    const double* partial1;
+    int single_row;
+};
+
 // Number of partial rows of particle i's tile (the CTAs first..last of the partition touch it).
 __device__ __forceinline__ int tile_slots(const PairPart& P, long long i) {
     long long first, last;
@@ -684,21 +703,26 @@ __device__ __forceinline__ int tile_slots(const PairPart& P, long long i) {
 template <int MODEL, bool KICK2, bool DRIFT>
 __global__ void __launch_bounds__(kUpdThreads)
 pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __restrict__ p0, double* __restrict__ p1,
-                   PairPart P, int fixed_slots, const double* __restrict__ partial0, const double* __restrict__ partial1,
-                   double kickA, double kickB, double drift, double2* __restrict__ js, float2* __restrict__ js32) {
+                   PairPart P, ForceRows FR, double kickA, double kickB, double drift, double2* __restrict__ js,
+                   float2* __restrict__ js32) {
     const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
-    const int S = fixed_slots > 0 ? fixed_slots : tile_slots(P, i);   // 1 after pair_sym_fold_kernel
-    double f = partial0[i];
-    for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
+    double f, g = 0.0;
+    {
+        const int S = FR.single_row ? 1 : tile_slots(P, i);
+        f = FR.partial0[i];
+        for (int s = 1; s < S; ++s) f += FR.partial0[(long long)s * N + i];
+        if (MODEL == 2) {
+            g = FR.partial1[i];
+            for (int s = 1; s < S; ++s) g += FR.partial1[(long long)s * N + i];
+        }
+    }
     double p = fma(kickA, f, p0[i]);
     if (KICK2) p = fma(kickB, f, p);
     p0[i] = p;
     double pb = 0.0;
     if (MODEL == 2) {
-        double g = partial1[i];
-        for (int s = 1; s < S; ++s) g += partial1[(long long)s * N + i];
         pb = fma(kickA, g, p1[i]);
         if (KICK2) pb = fma(kickB, g, pb);
         p1[i] = pb;
@@ -721,20 +745,22 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
 
 // lrmd_forces for the pair models: f = sum_s partial[s][i]
 __global__ void __launch_bounds__(kUpdThreads)
-pair_force_out_kernel(PairPart P, int fixed_slots, const double* __restrict__ partial0,
-                      const double* __restrict__ partial1, double* __restrict__ f0, double* __restrict__ f1) {
+pair_force_out_kernel(PairPart P, ForceRows FR, double* __restrict__ f0, double* __restrict__ f1) {
     const long long N = P.Ni;
     const long long i = (long long)blockIdx.x * kUpdThreads + threadIdx.x;
     if (i >= N) return;
-    const int S = fixed_slots > 0 ? fixed_slots : tile_slots(P, i);
-    double f = partial0[i];
-    for (int s = 1; s < S; ++s) f += partial0[(long long)s * N + i];
-    f0[i] = f;
-    if (f1) {
-        double g = partial1[i];
-        for (int s = 1; s < S; ++s) g += partial1[(long long)s * N + i];
-        f1[i] = g;
+    double f, g = 0.0;
+    {
+        const int S = FR.single_row ? 1 : tile_slots(P, i);
+        f = FR.partial0[i];
+        for (int s = 1; s < S; ++s) f += FR.partial0[(long long)s * N + i];
+        if (f1) {
+            g = FR.partial1[i];
+            for (int s = 1; s < S; ++s) g += FR.partial1[(long long)s * N + i];
+        }
     }
+    f0[i] = f;
+    if (f1) f1[i] = g;
 }
 
 }  // namespace lrmd
