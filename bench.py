@@ -150,7 +150,8 @@ def units_per_force(w):
     return "pair-interactions/s", "pair-interactions/s", float(w.N) * float(w.N)
 
 
-def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False, ordered_pairs=False):
+def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False, ordered_pairs=False,
+                 force_symmetric=False):
     import torch
     from paper_1212_0262_b200 import lrmd
 
@@ -159,7 +160,8 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     st = w.state()
     ctx = lrmd.Context(w.model, w.N, w.eps, device=dev,
                        options=({lrmd.OPT_PAIR_PRECISION: 1} if f32_pairs else
-                                ({lrmd.OPT_PAIR_SYMMETRIC: 0} if (ordered_pairs and w.model != 0) else None)))
+                                ({lrmd.OPT_PAIR_SYMMETRIC: 0} if (ordered_pairs and w.model != 0) else
+                                 ({lrmd.OPT_PAIR_SYMMETRIC: 1} if force_symmetric else None))))
     ctx.set_state(*st)
     stream = torch.cuda.current_stream(dev)
     state_bytes = ctx.narrays * w.N * 8
@@ -459,6 +461,14 @@ def main():
             others[key + "_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
                                                                  "options", "clocks", "roofline") if k in r}
             others[key + "_ordered_pairs"]["steps"] = DEFAULT_STEPS[key]
+        # config 5 with the symmetric kernel forced: its j-side scratch rows take 64 GiB of the 180 GB (opt-in only)
+        try:
+            r = run_workload(inputs.WORKLOADS["grav2d_1m"], 3, 3, None, with_e2e=False, force_symmetric=True)
+            others["grav2d_1m_symmetric_64GiB_scratch"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches",
+                                                                               "l2", "options", "clocks", "roofline") if k in r}
+            others["grav2d_1m_symmetric_64GiB_scratch"]["steps"] = 3
+        except Exception as e:      # e.g. not enough free HBM on a shared box: the default line does not depend on it
+            others["grav2d_1m_symmetric_64GiB_scratch"] = {"skipped": repr(e)[:200]}
         # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
         r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)
         others["grav2d_1m_f32pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
