@@ -237,6 +237,10 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         kms, kn = ctx.kernel_time()
         ctx.set_option(lrmd.OPT_KERNEL_TIMING, 0)
         avg_s = (kms / max(kn, 1)) * 1e-3
+        if w.model != 0:
+            # pair models: per FORCE EVALUATION (3 per step; the symmetric kernel may take several launches, one per
+            # batch of i-tiles, for one evaluation)
+            avg_s = (kms / (3.0 * Kr)) * 1e-3
         clk = (clocks.get("sm_mhz") or peaks["sm_max_mhz"])
         if w.model == 0:
             bytes_per_launch = HMF_BYTES_PER_PARTICLE_SUBSTAGE * w.N
@@ -276,6 +280,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         roof.update({"kernel": {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else
                                  ("pair_force_sym_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "pair_force_kernel")),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
+                     "kernel_launches_per_force_evaluation": (kn / (3.0 * Kr)) if w.model != 0 else None,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else "") +
                                                       ("_sym" if (w.model != 0 and not f32_pairs and
@@ -455,20 +460,12 @@ def main():
                                               "clocks", "roofline", "e2e", "energy") if k in r}
             others[key]["steps"] = DEFAULT_STEPS[key]
         # the paper's own scheme, every ORDERED pair, on the configs where the symmetric kernel is the default
-        for key in ("ring_16k", "grav2d_64k"):
+        for key in ("ring_16k", "grav2d_64k", "grav2d_1m"):
             ow = inputs.WORKLOADS[key]
-            r = run_workload(ow, DEFAULT_STEPS[key], 3, None, with_e2e=False, ordered_pairs=True)
+            r = run_workload(ow, 3 if key == "grav2d_1m" else DEFAULT_STEPS[key], 3, None, with_e2e=False, ordered_pairs=True)
             others[key + "_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
                                                                  "options", "clocks", "roofline") if k in r}
-            others[key + "_ordered_pairs"]["steps"] = DEFAULT_STEPS[key]
-        # config 5 with the symmetric kernel forced: its j-side scratch rows take 64 GiB of the 180 GB (opt-in only)
-        try:
-            r = run_workload(inputs.WORKLOADS["grav2d_1m"], 3, 3, None, with_e2e=False, force_symmetric=True)
-            others["grav2d_1m_symmetric_64GiB_scratch"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches",
-                                                                               "l2", "options", "clocks", "roofline") if k in r}
-            others["grav2d_1m_symmetric_64GiB_scratch"]["steps"] = 3
-        except Exception as e:      # e.g. not enough free HBM on a shared box: the default line does not depend on it
-            others["grav2d_1m_symmetric_64GiB_scratch"] = {"skipped": repr(e)[:200]}
+            others[key + "_ordered_pairs"]["steps"] = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]
         # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
         r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)
         others["grav2d_1m_f32pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",

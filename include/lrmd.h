@@ -76,11 +76,13 @@ enum {
     LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
                                     of the pair kernels (-1 = choose)                                          */
     LRMD_OPT_PAIR_SLOTS = 7,     /* read-only (lrmd_get_option): partial force rows per particle          */
-    LRMD_OPT_PAIR_SYMMETRIC = 8  /* pair models, fp64: 1 = force kernel that evaluates every UNORDERED pair once and adds
+    LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models, fp64: 1 = force kernel that evaluates every UNORDERED pair once and adds
                                     +f / -f to both particles (the paper declines this);
-                                    0 = every ordered pair (the paper's scheme); -1 = choose (symmetric when its
-                                    N x N/tile scratch rows fit 1 GiB and the context is not a shard).  With 1,
-                                    LRMD_OPT_PAIR_CTAS counts warps (workers), not CTAs.                          */
+                                    0 = every ordered pair (the paper's scheme); -1 = choose (symmetric for N >= 2048
+                                    unless the context is a shard or uses fp32 pair terms).  With the symmetric
+                                    kernel LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, not CTAs.            */
+    LRMD_OPT_PAIR_SYM_TILES = 9  /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
+                                    N doubles per tile and component, within 1 GiB); get: the value in use            */
 };
 
 /* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.

@@ -53,7 +53,7 @@ struct lrmd_ctx {
     void* coll_user = nullptr;
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
-    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1;
+    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0;
     // resolved
     int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
     int slots = 1;              // partial force rows per particle (pair models)
@@ -62,7 +62,8 @@ struct lrmd_ctx {
     lrmd::SymPart spart{};      // its work partition; the two tables below are uploaded by lrmd_set_workspace
     std::vector<int4> sym_wstart;
     std::vector<int2> sym_tiles;
-    int sym_slots = 1, sym_R = 4;
+    std::vector<int4> sym_batches;   // (first tile, end tile, first worker, workers) per launch
+    int sym_slots = 1, sym_R = 4, sym_rows = 1;
     bool use_graph = false;
     Layout lay;
     // bindings
@@ -100,6 +101,7 @@ constexpr int kHmfClusterVariant = 3;   // cluster-resident kernel: whole state 
 constexpr int64_t kHmfClusterMaxN = (int64_t)kHmfClusterCtas * kHmfClusterThreads * 4;   // 20,480
 constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
 constexpr int64_t kHmfTmaMinN = 1000000;
+constexpr double kSymRowBytes = 1073741824.0;   // scratch for the symmetric kernel's j-side rows per launch (1 GiB)
 
 // Pair kernels: <threads, i per thread, j per stage, CTAs per SM, j unroll>.
 using PairCfg0 = PairCfg<128, 4, 256, 4, 4>;   // Ring default (88 registers)
@@ -122,48 +124,61 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     c->sym = false;
     c->sym_wstart.clear();
     c->sym_tiles.clear();
+    c->sym_batches.clear();
     const int64_t N = c->N;
     if (c->opt_sym == 0 || c->N_total != c->N || c->opt_precision != 0) return;
+    if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
     const int R = c->pair_variant == 1 ? 8 : 4;
     const int T = 32 * R;
     const int64_t ntiles = (N + T - 1) / T, nchunks = (N + 31) / 32;
     const int comps = c->model == LRMD_GRAV2D ? 2 : 1;
-    const double jbytes = (double)ntiles * (double)N * 8.0 * comps;
-    // the j-side rows cost ntiles x N doubles per component: automatic only up to 1 GiB, on request up to 64 GiB
-    if (jbytes > (c->opt_sym == 1 ? 64.0 : 1.0) * 1073741824.0) return;
-    if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
-    int64_t U = 0;
-    for (int64_t a = 0; a < ntiles; ++a) U += nchunks - a * R;
-    // workers: R = 4 (80 registers) keeps 24 warps per SM resident, R = 8 (138 registers) 12; measured best at
-    // 32 and 12 workers per SM (profiles/); at least two units per worker
-    int64_t G = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * (R == 8 ? 12 : 32);
-    if (c->opt_pair_ctas <= 0 && G > U / 2) G = U / 2;
-    if (G > U) G = U;
-    if (G < 1) G = 1;
-    c->sym_wstart.resize((size_t)G);
+    // The j-side rows cost N doubles per component and tile.  Tiles are processed in batches of TB tiles (one
+    // kernel launch + one fold per batch) so that the rows of a batch fit kSymRowBytes: one batch up to
+    // N ~ 1.8e5 (2D), 64 batches at N = 2^20.
+    int64_t TB = (int64_t)(kSymRowBytes / ((double)N * 8.0 * comps));
+    if (c->opt_sym_tiles > 0) TB = c->opt_sym_tiles;
+    if (TB < 1) TB = 1;
+    if (TB > ntiles) TB = ntiles;
+    // workers per launch: R = 4 (80 registers) keeps 24 warps per SM resident, R = 8 (138 registers) 12; measured
+    // best at 32 and 12 workers per SM (profiles/); at least two units per worker
+    const int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * (R == 8 ? 12 : 32);
     c->sym_tiles.assign((size_t)ntiles, make_int2(0x7fffffff, -1));
-    int64_t a = 0, cum = 0;     // cum = units before tile a
-    for (int64_t w = 0; w < G; ++w) {
-        const int64_t u0 = (w * U) / G, u1 = ((w + 1) * U) / G;
-        while (u0 >= cum + (nchunks - a * R)) { cum += nchunks - a * R; ++a; }
-        c->sym_wstart[(size_t)w] = make_int4((int)a, (int)(a * R + (u0 - cum)), (int)(u1 - u0), 0);
-        // tiles this worker touches
-        int64_t aa = a, cc = cum;
-        for (;;) {
-            int2& r = c->sym_tiles[(size_t)aa];
-            if ((int)w < r.x) r.x = (int)w;
-            if ((int)w > r.y) r.y = (int)w;
-            if (u1 <= cc + (nchunks - aa * R)) break;
-            cc += nchunks - aa * R;
-            ++aa;
+    int gmax = 1;
+    for (int64_t t0 = 0; t0 < ntiles; t0 += TB) {
+        const int64_t t1 = t0 + TB < ntiles ? t0 + TB : ntiles;
+        int64_t U = 0;
+        for (int64_t a = t0; a < t1; ++a) U += nchunks - a * R;
+        int64_t G = Gwant;
+        if (c->opt_pair_ctas <= 0 && G > U / 2) G = U / 2;
+        if (G > U) G = U;
+        if (G < 1) G = 1;
+        const int64_t w0 = (int64_t)c->sym_wstart.size();
+        c->sym_batches.push_back(make_int4((int)t0, (int)t1, (int)w0, (int)G));
+        if (G > gmax) gmax = (int)G;
+        int64_t a = t0, cum = 0;     // cum = units of the batch before tile a
+        for (int64_t w = 0; w < G; ++w) {
+            const int64_t u0 = (w * U) / G, u1 = ((w + 1) * U) / G;
+            while (u0 >= cum + (nchunks - a * R)) { cum += nchunks - a * R; ++a; }
+            c->sym_wstart.push_back(make_int4((int)a, (int)(a * R + (u0 - cum)), (int)(u1 - u0), 0));
+            const int gw = (int)(w0 + w);     // global worker index: slots are counted from a tile's first worker
+            int64_t aa = a, cc = cum;
+            for (;;) {
+                int2& r = c->sym_tiles[(size_t)aa];
+                if (gw < r.x) r.x = gw;
+                if (gw > r.y) r.y = gw;
+                if (u1 <= cc + (nchunks - aa * R)) break;
+                cc += nchunks - aa * R;
+                ++aa;
+            }
         }
     }
     int smax = 1;
     for (const int2& r : c->sym_tiles) if (r.y - r.x + 1 > smax) smax = r.y - r.x + 1;
     c->sym_slots = smax;
     c->sym_R = R;
+    c->sym_rows = (int)TB;
     lrmd::SymPart S;
-    S.N = N; S.T = T; S.ntiles = (int)ntiles; S.nchunks = (int)nchunks; S.G = (int)G;
+    S.N = N; S.T = T; S.ntiles = (int)ntiles; S.nchunks = (int)nchunks; S.G = gmax; S.w0 = 0; S.tile0 = 0; S.tile1 = (int)ntiles;
     S.wstart = nullptr; S.tile_rng = nullptr;
     c->spart = S;
     c->sym = true;
@@ -246,8 +261,8 @@ void resolve(lrmd_ctx* c) {
             L.sym_tiles = off; off = align_up(off + sizeof(int2) * c->sym_tiles.size());
             L.ipart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots);
             if (two) { L.ipart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots); }
-            L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->spart.ntiles);
-            if (two) { L.jpart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->spart.ntiles); }
+            L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows);
+            if (two) { L.jpart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows); }
         }
         L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
         c->use_graph = false;
@@ -553,24 +568,28 @@ void pair_pack(Launcher& L) {
 
 inline double* wsd(lrmd_ctx* c, size_t off) { return off ? reinterpret_cast<double*>(c->ws + off) : nullptr; }
 
-// Symmetric force evaluation (row N4) + the fold into one force row.
+// Symmetric force evaluation (row N4): per batch of tiles one kernel launch + the fold into the force row.
 void pair_force_sym(Launcher& L) {
     lrmd_ctx* c = L.c;
-    const dim3 g((unsigned)((c->spart.G + kSymThreads / 32 - 1) / (kSymThreads / 32))), b(kSymThreads);
     double *i0 = wsd(c, c->lay.ipart0), *i1 = wsd(c, c->lay.ipart1), *j0 = wsd(c, c->lay.jpart0), *j1 = wsd(c, c->lay.jpart1);
-    if (c->model == LRMD_RING) {
-        const double pre = -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N);
-        if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<1, 8>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
-        else L.go_timed(pair_force_sym_kernel<1, 4>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
-    } else {
-        const double pre = -2.0 / (double)c->N;
-        if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<2, 8>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
-        else L.go_timed(pair_force_sym_kernel<2, 4>, g, b, js_ptr(c), c->spart, c->eps, pre, i0, i1, j0, j1);
+    const double pre = c->model == LRMD_RING ? -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N) : -2.0 / (double)c->N;
+    for (const int4& bt : c->sym_batches) {
+        SymPart S = c->spart;
+        S.tile0 = bt.x; S.tile1 = bt.y; S.w0 = bt.z; S.G = bt.w;
+        const dim3 g((unsigned)((S.G + kSymThreads / 32 - 1) / (kSymThreads / 32))), b(kSymThreads);
+        if (c->model == LRMD_RING) {
+            if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<1, 8>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
+            else L.go_timed(pair_force_sym_kernel<1, 4>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
+        } else {
+            if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<2, 8>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
+            else L.go_timed(pair_force_sym_kernel<2, 4>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
+        }
+        // rows of this batch only concern particles from its first tile on
+        const long long first = (long long)S.tile0 * S.T;
+        L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N - first + 31) / 32)), dim3(32, 8), S, (const double*)i0,
+             (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
     }
-    L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N + 31) / 32)), dim3(32, 8), c->spart, (const double*)i0,
-         (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
 }
-
 
 ForceRows force_rows(lrmd_ctx* c) {
     ForceRows FR;
@@ -894,6 +913,11 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
             c->opt_sym = value;
             break;
+        case LRMD_OPT_PAIR_SYM_TILES:
+            if (value < 0 || value > (1 << 24)) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
+            c->opt_sym_tiles = value;
+            break;
         case LRMD_OPT_KERNEL_TIMING:
             if (value != 0 && value != 1) return LRMD_EINVAL;
             c->timing = value != 0;
@@ -920,6 +944,7 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
         case LRMD_OPT_PAIR_VARIANT: *value = c->pair_variant; break;
         case LRMD_OPT_PAIR_SLOTS: *value = c->sym ? c->sym_slots : c->slots; break;
         case LRMD_OPT_PAIR_SYMMETRIC: *value = c->sym ? 1 : 0; break;
+        case LRMD_OPT_PAIR_SYM_TILES: *value = c->sym ? c->sym_rows : 0; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;

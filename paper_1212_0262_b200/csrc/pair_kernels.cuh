@@ -376,9 +376,11 @@ struct SymPart {
     int T;            // particles per i-tile = 32 R
     int ntiles;       // ceil(N / T)
     int nchunks;      // ceil(N / 32)
-    int G;            // workers (warps)
-    const int4* wstart;    // [G]  first unit of worker w: (tile, chunk, number of units, 0)
-    const int2* tile_rng;  // [ntiles] first and last worker touching the tile
+    int G;            // workers (warps) of this launch
+    int w0;           // index of this launch's first worker in wstart (launches = batches of tiles tile0 .. tile1 - 1,
+    int tile0, tile1; //   so that the j-side rows of one launch fit their scratch: jpart[tile - tile0][j])
+    const int4* wstart;    // first unit of every worker: (tile, chunk, number of units, 0)
+    const int2* tile_rng;  // [ntiles] first and last (global) worker touching the tile
 };
 
 constexpr int kSymThreads = 128;   // 4 independent workers per CTA
@@ -440,7 +442,7 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
     const int lane = threadIdx.x & 31;
     const long long N = S.N;
     const double onepe = 1.0 + eps;
-    const int4 st = S.wstart[w];
+    const int4 st = S.wstart[S.w0 + w];
     int tile = st.x, chunk = st.y;
     const bool ragged = (N % S.T) != 0 || (N % 32) != 0;
 
@@ -460,7 +462,7 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
         }
     };
     auto store_tile = [&](int t) {
-        const int slot = w - S.tile_rng[t].x;
+        const int slot = S.w0 + w - S.tile_rng[t].x;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long i = (long long)t * S.T + r * 32 + lane;
@@ -504,8 +506,8 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
             if (masked) sym_chunk<MODEL, R, true, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
             else sym_chunk<MODEL, R, false, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
             if (vq) {
-                jpart0[(long long)ctile * N + j] = pre * g0;
-                if (MODEL == 2) jpart1[(long long)ctile * N + j] = pre * g1;
+                jpart0[(long long)(ctile - S.tile0) * N + j] = pre * g0;
+                if (MODEL == 2) jpart1[(long long)(ctile - S.tile0) * N + j] = pre * g1;
             }
         }
         if (tile_done || !more) {
@@ -648,27 +650,32 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
     }
 }
 
-// Symmetric kernel's result for particle i: the i-side rows of the workers that touched i's tile + the j-side
-// rows of all lower tiles -> out0 / out1 (one force row).  Block = 32 particles x 8 row groups: group k adds
-// the rows k, k + 8, ... of each list in order, the 8 group sums are combined in a fixed tree: deterministic,
-// and eight times shorter than one dependent chain of ~100 loads per particle.
+// Folds one launch (batch of tiles tile0 .. tile1 - 1) of the symmetric kernel into the force row out0 / out1:
+// for particle i (from the batch's first particle on) the i-side rows of the workers that touched i's tile, if the
+// tile is in the batch, + the j-side rows of the batch's tiles below i's tile.  The first batch writes, later ones
+// add (batches run in tile order on one stream).  Block = 32 particles x 8 row groups: group k adds the rows
+// k, k + 8, ... of each list in order, the 8 group sums are combined in a fixed tree: deterministic, and eight
+// times shorter than one dependent chain of ~100 loads per particle.
 __global__ void __launch_bounds__(256)
 pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
                      const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
                      double* __restrict__ out1) {
     __shared__ double sf[8][32], sg[8][32];
     const long long N = S.N;
-    const long long i = (long long)blockIdx.x * 32 + threadIdx.x;
+    const long long i = (long long)S.tile0 * S.T + (long long)blockIdx.x * 32 + threadIdx.x;
     const int k = threadIdx.y;
     double f = 0.0, g = 0.0;
     if (i < N) {
         const int t = (int)(i / S.T);
-        const int2 rng = S.tile_rng[t];
-        for (int s = k; s <= rng.y - rng.x; s += 8) {
-            f += ipart0[(long long)s * N + i];
-            if (ipart1) g += ipart1[(long long)s * N + i];
+        if (t < S.tile1) {
+            const int2 rng = S.tile_rng[t];
+            for (int s = k; s <= rng.y - rng.x; s += 8) {
+                f += ipart0[(long long)s * N + i];
+                if (ipart1) g += ipart1[(long long)s * N + i];
+            }
         }
-        for (int a = k; a < t; a += 8) {
+        const int nrows = (t < S.tile1 ? t : S.tile1) - S.tile0;     // batch tiles below i's tile
+        for (int a = k; a < nrows; a += 8) {
             f += jpart0[(long long)a * N + i];
             if (jpart1) g += jpart1[(long long)a * N + i];
         }
@@ -678,8 +685,15 @@ pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double*
     __syncthreads();
     if (k == 0 && i < N) {
         const int x = threadIdx.x;
-        out0[i] = ((sf[0][x] + sf[1][x]) + (sf[2][x] + sf[3][x])) + ((sf[4][x] + sf[5][x]) + (sf[6][x] + sf[7][x]));
-        if (out1) out1[i] = ((sg[0][x] + sg[1][x]) + (sg[2][x] + sg[3][x])) + ((sg[4][x] + sg[5][x]) + (sg[6][x] + sg[7][x]));
+        const double ff = ((sf[0][x] + sf[1][x]) + (sf[2][x] + sf[3][x])) + ((sf[4][x] + sf[5][x]) + (sf[6][x] + sf[7][x]));
+        const double gg = ((sg[0][x] + sg[1][x]) + (sg[2][x] + sg[3][x])) + ((sg[4][x] + sg[5][x]) + (sg[6][x] + sg[7][x]));
+        if (S.tile0 == 0) {
+            out0[i] = ff;
+            if (out1) out1[i] = gg;
+        } else {
+            out0[i] += ff;
+            if (out1) out1[i] += gg;
+        }
     }
 }
 

@@ -18,7 +18,7 @@ import os
 HMF, RING, GRAV2D = 0, 1, 2
 OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED, ECOLL = 0, -1, -2, -3, -4, -5
 OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
-OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS, OPT_PAIR_SYMMETRIC = 5, 6, 7, 8
+OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS, OPT_PAIR_SYMMETRIC, OPT_PAIR_SYM_TILES = 5, 6, 7, 8, 9
 
 #: every symbol include/lrmd.h declares (tests check the library exports each of them)
 SYMBOLS = (

@@ -430,6 +430,33 @@ def test_symmetric_force_kernel_matches_oracle(lrmd, ref, torch, model, N, varia
 
 
 @pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("tiles", [1, 3, 7])
+def test_symmetric_kernel_in_batches_of_tiles(lrmd, ref, torch, model, tiles):
+    """Several launches per force evaluation (the j-side scratch rows of one launch are bounded): each batch's
+    fold adds to the force row in tile order."""
+    eps = _eps(model)
+    N = 3001
+    st = _state(model, N, 4242)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_SYMMETRIC: 1, lrmd.OPT_PAIR_SYM_TILES: tiles})
+    assert ctx.get_option(lrmd.OPT_PAIR_SYM_TILES) == tiles
+    ctx.set_state(*st)
+    f = ctx.forces()
+    got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    _check_forces(model, got, (f0, f1), (A0, A1))
+    ctx.step(4, 0.01)
+    out = ctx.state_numpy()
+    ctx.close()
+    r = [a.copy() for a in st]
+    rq0, rq1 = _q(model, r)
+    rp0, rp1 = _p(model, r)
+    ref.step(model, eps, rq0, rq1, rp0, rp1, 4, 0.01, form=1)
+    for g, w in zip(out, r):
+        assert np.max(np.abs(g - w)) <= XTOL
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
 def test_symmetric_kernel_trajectory_momentum_and_reproducibility(lrmd, ref, torch, model):
     eps = _eps(model)
     N = 5001
@@ -459,9 +486,12 @@ def test_symmetric_default_choice(lrmd, torch):
     b = lrmd.Context(GRAV2D, 65_536, 1e-3)
     c = lrmd.Context(GRAV2D, 1_048_576, 1e-3)
     d = lrmd.Context(GRAV2D, 65_536, 1e-3, options={lrmd.OPT_PAIR_SYMMETRIC: 0})
+    e = lrmd.Context(GRAV2D, 1000, 1e-3)
     assert a.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and b.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
-    assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0      # 64 GiB of j-side rows: the ordered kernel stays
-    assert d.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0
+    assert b.get_option(lrmd.OPT_PAIR_SYM_TILES) == 256     # all 256 tiles in one launch (268 MB of j-side rows)
+    assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and c.get_option(lrmd.OPT_PAIR_SYM_TILES) == 64   # 64 launches of 64 tiles
+    assert d.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0 and e.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0
+    e.close()
     for x in (a, b, c, d):
         x.close()
 
