@@ -399,28 +399,64 @@ __device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b
         const double qny = __shfl_sync(0xffffffffu, q.y, src);
         const bool vqn = MASK ? (__shfl_sync(0xffffffffu, (int)vq, src) != 0) : true;
         double h0 = 0.0, h1 = 0.0;
+        // The R pair evaluations of a step are written stage by stage over groups of 4, so that the four
+        // dependency chains (difference -> r^2 -> MUFU seed -> correction -> accumulate) are interleaved in
+        // the instruction stream: written pair by pair, the compiler reused one register set and ran the
+        // chains back to back, every correction waiting for its own seed (profiles/r01e_summary.md).
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
+        for (int r0 = 0; r0 < R; r0 += 4) {
             if (MODEL == 2) {
-                const double dx = a[r] - q.x, dy = b[r] - q.y;
-                const double r2 = fma(dy, dy, fma(dx, dx, eps));
-                const double y0 = rcp_seed(r2);
-                const double e = fma(-r2, y0, 1.0);
-                const double t = fma(e, e, e);
-                double y = fma(y0, t, y0);
-                if (MASK) y = (vi[r] && vq) ? y : 0.0;
-                f0[r] = fma(dx, y, f0[r]);
-                f1[r] = fma(dy, y, f1[r]);
-                if (!DIAG) {
-                    h0 = fma(-dx, y, h0);
-                    h1 = fma(-dy, y, h1);
+                double dx[4], dy[4], r2[4], y0[4], y[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    dx[k] = a[r0 + k] - q.x;
+                    dy[k] = b[r0 + k] - q.y;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) r2[k] = fma(dy[k], dy[k], fma(dx[k], dx[k], eps));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y0[k] = rcp_seed(r2[k]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double e = fma(-r2[k], y0[k], 1.0);
+                    y[k] = fma(e, e, e);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    y[k] = fma(y0[k], y[k], y0[k]);
+                    if (MASK) y[k] = (vi[r0 + k] && vq) ? y[k] : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    f0[r0 + k] = fma(dx[k], y[k], f0[r0 + k]);
+                    f1[r0 + k] = fma(dy[k], y[k], f1[r0 + k]);
+                    if (!DIAG) {
+                        h0 = fma(-dx[k], y[k], h0);
+                        h1 = fma(-dy[k], y[k], h1);
+                    }
                 }
             } else {
-                double c, p;
-                ring_pair_parts(a[r], b[r], q, onepe, c, p);
-                if (MASK) c = (vi[r] && vq) ? c : 0.0;
-                f0[r] = fma(c, p, f0[r]);
-                if (!DIAG) h0 = fma(-c, p, h0);
+                double num[4], d[4], y0[4], c[4], p[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    num[k] = fma(b[r0 + k], q.x, -(a[r0 + k] * q.y));                 // s_i c_j - c_i s_j
+                    d[k] = fma(-b[r0 + k], q.y, fma(-a[r0 + k], q.x, onepe));      // 1 + eps - c_i c_j - s_i s_j
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y0[k] = rsqrt_seed(d[k]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double bb = y0[k] * y0[k];
+                    const double e = fma(-d[k], bb, 1.0);
+                    c[k] = (num[k] * y0[k]) * bb;
+                    p[k] = fma(fma(1.875, e, 1.5), e, 1.0);
+                    if (MASK) c[k] = (vi[r0 + k] && vq) ? c[k] : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    f0[r0 + k] = fma(c[k], p[k], f0[r0 + k]);
+                    if (!DIAG) h0 = fma(-c[k], p[k], h0);
+                }
             }
         }
         if (!DIAG) {
