@@ -192,6 +192,13 @@ int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_
  * *nseg_host: the CTA adds the pairs (i in tile) x (jbeg <= j < jend) into partial force row `slot`. */
 int lrmd_pair_partition(const lrmd_ctx* ctx, int64_t cta, int64_t* seg4_host, int64_t max_seg, int64_t* nseg_host);
 
+/* Diagnostic (HOST pointers, no GPU needed): the work table of the symmetric pair kernel (LRMD_OPT_PAIR_SYMMETRIC).
+ * Work units are (i-tile, chunk of 32 j) pairs with chunk >= tile * (tile size / 32), in tile-major order; each
+ * launch (batch of consecutive tiles) divides its units evenly over its workers (warps).  *n_workers_host (if not
+ * NULL) receives the total number of workers over all launches (0 if the symmetric kernel is not in use);
+ * out5_host (if not NULL) receives {tile, chunk, units, launch, tile size} of worker `worker`. */
+int lrmd_pair_sym_partition(const lrmd_ctx* ctx, int64_t worker, int64_t* out5_host, int64_t* n_workers_host);
+
 #ifdef __cplusplus
 }
 #endif

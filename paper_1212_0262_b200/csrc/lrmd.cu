@@ -1017,6 +1017,23 @@ int lrmd_pair_partition(const lrmd_ctx* c, int64_t cta, int64_t* seg4_host, int6
     return LRMD_OK;
 }
 
+int lrmd_pair_sym_partition(const lrmd_ctx* c, int64_t worker, int64_t* out5_host, int64_t* n_workers_host) {
+    if (!c || c->model == LRMD_HMF) return LRMD_EINVAL;
+    if (n_workers_host) *n_workers_host = c->sym ? (int64_t)c->sym_wstart.size() : 0;
+    if (!out5_host) return n_workers_host ? LRMD_OK : LRMD_EINVAL;
+    if (!c->sym || worker < 0 || worker >= (int64_t)c->sym_wstart.size()) return LRMD_EINVAL;
+    const int4 st = c->sym_wstart[(size_t)worker];
+    int64_t batch = 0;
+    for (size_t b = 0; b < c->sym_batches.size(); ++b)
+        if (worker >= c->sym_batches[b].z && worker < c->sym_batches[b].z + c->sym_batches[b].w) batch = (int64_t)b;
+    out5_host[0] = st.x;                   // first unit: tile
+    out5_host[1] = st.y;                   //             chunk of 32 j
+    out5_host[2] = st.z;                   // number of (tile, chunk) units, tile-major
+    out5_host[3] = batch;                  // launch (batch of tiles) the worker belongs to
+    out5_host[4] = 32 * c->sym_R;          // particles per i-tile
+    return LRMD_OK;
+}
+
 int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host) {
     if (!x_host || !s_host || !c_host || n < 0) return LRMD_EINVAL;
     for (int64_t i = 0; i < n; ++i) sincos_any(x_host[i], s_host[i], c_host[i]);

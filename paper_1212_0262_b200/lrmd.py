@@ -25,7 +25,7 @@ SYMBOLS = (
     "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
-    "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard",
+    "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard", "lrmd_pair_sym_partition",
 )
 
 _lib = None
@@ -78,6 +78,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_pair_partition.argtypes = [_vp, _i64, _vp, _i64, C.POINTER(_i64)]
     lib.lrmd_step_observe.argtypes = [_vp, _i64, _dbl, _i64, _vp, _vp]
     lib.lrmd_set_shard.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp]
+    lib.lrmd_pair_sym_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int
@@ -200,6 +201,20 @@ def lrmd_pair_partition(ctx, cta: int, max_seg: int = 64):
     if rc == OK and n.value > max_seg:
         return lrmd_pair_partition(ctx, cta, int(n.value))
     return rc, buf[: n.value].copy()
+
+
+def lrmd_pair_sym_partition(ctx):
+    """Diagnostic: (rc, table) with one row {tile, chunk, units, launch, tile size} per worker of the symmetric
+    pair kernel (an empty table if it is not in use)."""
+    import numpy as np
+    n = _i64(0)
+    rc = load().lrmd_pair_sym_partition(ctx, 0, None, C.byref(n))
+    tab = np.zeros((n.value, 5), dtype=np.int64)
+    for w in range(n.value):
+        if rc != OK:
+            break
+        rc = load().lrmd_pair_sym_partition(ctx, w, tab[w].ctypes.data, None)
+    return rc, tab
 
 
 # ---- convenience object ---------------------------------------------------------------------------------

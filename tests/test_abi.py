@@ -165,6 +165,57 @@ def test_pair_partition_covers_every_pair_once(lrmd, model, N, G):
     lrmd.lrmd_destroy(h)
 
 
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N,workers,tiles,variant", [(2048, 0, 0, -1), (5000, 7, 0, 0), (5000, 0, 3, 1), (16_384, 0, 0, -1),
+                                                     (65_536, 0, 0, -1), (33, 5, 1, 0), (1000, 1, 0, 1), (300_001, 0, 0, -1)])
+def test_symmetric_work_table_covers_every_unit_once(lrmd, model, N, workers, tiles, variant):
+    """Host logic of the symmetric pair kernel: every (tile, chunk >= first chunk of the tile) unit
+    belongs to exactly one worker, in tile-major order; launches take consecutive tiles; inside a launch the
+    workers' unit counts differ by at most one."""
+    rc, h = lrmd.lrmd_create(model, N, 1e-3)
+    assert rc == lrmd.OK
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 1) == lrmd.OK
+    if variant >= 0:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_VARIANT, variant) == lrmd.OK
+    if workers:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, workers) == lrmd.OK
+    if tiles:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYM_TILES, tiles) == lrmd.OK
+    rc, tab = lrmd.lrmd_pair_sym_partition(h)
+    assert rc == lrmd.OK and len(tab) >= 1
+    T = int(tab[0, 4])
+    R = T // 32
+    assert T == (128 if variant == 0 else 256)
+    ntiles, nchunks = -(-N // T), -(-N // 32)
+    tile, chunk = 0, 0                     # the unit the next worker must start with
+    launch, per_launch = 0, {}
+    for t0, c0, units, b, _ in tab:
+        assert (t0, c0) == (tile, chunk) and units >= 1
+        assert b in (launch, launch + 1)
+        if b == launch + 1:
+            assert chunk == tile * R        # a launch starts at the beginning of a tile
+            launch = b
+        per_launch.setdefault(int(b), []).append(int(units))
+        for _ in range(int(units)):
+            assert tile < ntiles and tile * R <= chunk < nchunks
+            chunk += 1
+            if chunk == nchunks:
+                tile += 1
+                chunk = tile * R
+    assert tile == ntiles                  # all units consumed, nothing left over
+    for b, us in per_launch.items():
+        assert max(us) - min(us) <= 1
+        if workers:
+            assert len(us) <= workers
+    if tiles:
+        assert len(per_launch) == -(-ntiles // tiles)
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(model, 100, 1e-3)          # below 2048 the ordered kernel is chosen: empty table
+    rc, tab = lrmd.lrmd_pair_sym_partition(h)
+    assert rc == lrmd.OK and len(tab) == 0
+    lrmd.lrmd_destroy(h)
+
+
 def test_strerror_and_coefficients(lrmd):
     assert lrmd.strerror(0) == "ok"
     for code in (-1, -2, -3, -4, -77):
