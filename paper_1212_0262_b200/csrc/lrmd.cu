@@ -128,7 +128,8 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     const int64_t N = c->N;
     if (c->opt_sym == 0 || c->N_total != c->N || c->opt_precision != 0) return;
     if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
-    const int R = c->opt_pair_variant == 0 ? 4 : 8;     // 8 i per lane unless launch shape 0 is asked for
+    // i per lane: Ring 4, 2D 8 (sweeps, profiles/); launch shape 0 / 1 asks for 4 / 8
+    const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
     const int T = 32 * R;
     const int64_t ntiles = (N + T - 1) / T, nchunks = (N + 31) / 32;
     const int comps = c->model == LRMD_GRAV2D ? 2 : 1;
@@ -139,10 +140,9 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     if (c->opt_sym_tiles > 0) TB = c->opt_sym_tiles;
     if (TB < 1) TB = 1;
     if (TB > ntiles) TB = ntiles;
-    // workers per launch, from sweeps (profiles/): R = 8 (140 registers, 12 warps per SM resident) 12 per SM for 2D
-    // and 16 for Ring, R = 4 (80 registers) 32; at least two units per worker
+    // workers per launch: 32 per SM (4 waves of the 8 resident warps; sweeps in profiles/); at least two units each
     const int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas
-                          : (int64_t)kNumSm * (R == 8 ? (c->model == LRMD_RING ? 16 : 12) : 32);
+                          : (int64_t)kNumSm * 32;
     c->sym_tiles.assign((size_t)ntiles, make_int2(0x7fffffff, -1));
     int gmax = 1;
     for (int64_t t0 = 0; t0 < ntiles; t0 += TB) {
