@@ -56,7 +56,7 @@ HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 NCU_TRAFFIC_BYTES = {"ring_16k": 279808.0, "grav2d_64k": 1067264.0, "hmf_5e7": 1541759232.0, "grav2d_1m": None,
                      "hmf_1e4": None, "grav2d_64k_f32": 554240.0,
                      # symmetric kernel (profiles/r01f_summary.md): j-stream reads + the j-side rows it writes
-                     "ring_16k_sym": 366592.0, "grav2d_64k_sym": 85512448.0}
+                     "ring_16k_sym": 404480.0, "grav2d_64k_sym": 98298368.0}
 
 DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5}
 
