@@ -94,7 +94,7 @@ def test_forces_any_partition(lrmd, ref, torch, model, S):
     st = _state(model, N, 77)
     q0, q1 = _q(model, st)
     f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
-    got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_PAIR_CTAS: S})
+    got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_PAIR_SYMMETRIC: 0, lrmd.OPT_PAIR_CTAS: S})
     _check_forces(model, got, (f0, f1), (A0, A1))
 
 
@@ -226,12 +226,13 @@ def test_forces_other_softenings(lrmd, ref, torch, model, eps):
     st = _state(model, N, 31)
     q0, q1 = _q(model, st)
     f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
-    got = _gpu_forces(lrmd, model, eps, st)
     if model == RING and eps < 0.01:
         # eq.(9)'s denominator cancels to ~eps for close pairs: relative rounding 2^-53/eps per pair,
         # x1.5 in d^(-3/2) (same allowance as the oracle's own eq.(8)-vs-eq.(9) pin)
         A0 = A0 * max(1.0, 1.5 * 4e-16 / eps / FTOL)
-    _check_forces(model, got, (f0, f1), (A0, A1))
+    for sym in (0, 1):     # the ordered kernel and the symmetric one
+        got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_PAIR_SYMMETRIC: sym})
+        _check_forces(model, got, (f0, f1), (A0, A1))
 
 
 def test_forces_coincident_particles(lrmd, ref, torch):
@@ -243,8 +244,9 @@ def test_forces_coincident_particles(lrmd, ref, torch):
             a[300:] = a[:300]
         q0, q1 = _q(model, st)
         f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
-        got = _gpu_forces(lrmd, model, eps, st)
-        _check_forces(model, got, (f0, f1), (A0, A1))
+        for sym in (0, 1):
+            got = _gpu_forces(lrmd, model, eps, st, options={lrmd.OPT_PAIR_SYMMETRIC: sym})
+            _check_forces(model, got, (f0, f1), (A0, A1))
 
 
 # ---- the BASELINE.json configs at full size -----------------------------------------------------------
@@ -349,13 +351,16 @@ def test_config4_hmf_5e7_sampled_and_invariants(lrmd, ref, torch, inputs):
     ctx.close()
 
 
-def test_config5_grav2d_1m_sampled_rows(lrmd, ref, torch, inputs):
-    """Config 5 at full size: forces on sampled rows (each against all N) at t = 0 and at the GPU's
-    positions after one step."""
+@pytest.mark.parametrize("symmetric", [-1, 0])
+def test_config5_grav2d_1m_sampled_rows(lrmd, ref, torch, inputs, symmetric):
+    """Config 5 at full size, in the launch configuration bench.py times (default: symmetric kernel in 64 launches
+    per force evaluation) and with the ordered kernel: forces on sampled rows (each against all N) at t = 0 and at
+    the GPU's positions after one step."""
     w = inputs.WORKLOADS["grav2d_1m"]
     x, y, px, py = w.state()
     rows = np.random.default_rng(6).choice(w.N, 512, replace=False)
-    ctx = lrmd.Context(GRAV2D, w.N, w.eps)
+    ctx = lrmd.Context(GRAV2D, w.N, w.eps, options={lrmd.OPT_PAIR_SYMMETRIC: symmetric})
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == (1 if symmetric else 0)
     ctx.set_state(x, y, px, py)
     fx, fy = (t.cpu().numpy() for t in ctx.forces())
     f0, f1, A0, A1 = ref.forces_rows(GRAV2D, w.eps, x, y, rows, with_abs=True)
