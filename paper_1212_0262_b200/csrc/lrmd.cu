@@ -265,7 +265,7 @@ void resolve(lrmd_ctx* c) {
             L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows);
             if (two) { L.jpart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows); }
         }
-        L.vpart = off; off = align_up(off + sizeof(double) * (size_t)G);
+        L.vpart = off; off = align_up(off + sizeof(double) * (c->sym && c->sym_wstart.size() > (size_t)G ? c->sym_wstart.size() : (size_t)G));
         c->use_graph = false;
     }
     L.kpart = off; off = align_up(off + sizeof(double) * 3 * kEnergyGrid);
@@ -822,6 +822,25 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
              hmf_sums(c, c->cur), hmf_nsums(c), (const double*)nullptr, 0, out4_device);
     } else {
         if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
+        if (c->sym) {
+            // V = pre * sum_{i<j} t_ij, every unordered pair evaluated once
+            const double pre = c->model == LRMD_RING ? -1.0 / (std::sqrt(2.0) * (double)c->N) : 1.0 / (double)c->N;
+            for (const int4& bt : c->sym_batches) {
+                SymPart S = c->spart;
+                S.tile0 = bt.x; S.tile1 = bt.y; S.w0 = bt.z; S.G = bt.w;
+                const dim3 g((unsigned)((S.G + kSymThreads / 32 - 1) / (kSymThreads / 32))), b(kSymThreads);
+                if (c->model == LRMD_RING) {
+                    if (c->sym_R == 8) L.go(pair_energy_sym_kernel<1, 8>, g, b, (const double2*)js_ptr(c), S, c->eps, pre, vpart(c));
+                    else L.go(pair_energy_sym_kernel<1, 4>, g, b, (const double2*)js_ptr(c), S, c->eps, pre, vpart(c));
+                } else {
+                    if (c->sym_R == 8) L.go(pair_energy_sym_kernel<2, 8>, g, b, (const double2*)js_ptr(c), S, c->eps, pre, vpart(c));
+                    else L.go(pair_energy_sym_kernel<2, 4>, g, b, (const double2*)js_ptr(c), S, c->eps, pre, vpart(c));
+                }
+            }
+            L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
+                 (const double2*)nullptr, 0, (const double*)vpart(c), (int)c->sym_wstart.size(), out4_device);
+            return L.rc;
+        }
         // V = pre * sum_{i<j} t_ij = (pre/2) * sum_{i != j} t_ij
         with_pair_cfg(c->pair_variant, [&](auto cfg) {
             using CFG = decltype(cfg);

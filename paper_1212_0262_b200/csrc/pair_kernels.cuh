@@ -667,6 +667,115 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
     if (threadIdx.x == 0) vpart[blockIdx.x] = pre_half * v[0];
 }
 
+// ---- symmetric potential-energy kernel -------------------------------------------------------------------------
+// V is a sum over unordered pairs to begin with (eqs.(1),(3): sum_{i<j}), so the walk of the symmetric force kernel
+// gives it with every pair evaluated once and nothing to send back: only the packet's position travels.  The chunks
+// of a tile itself count a pair only if j > i (masked walk, a small fraction of the units).  Worker w writes
+// vpart[w0 + w] = pre * (its sum over its units), lanes combined by the fixed shuffle tree; energy_finalize_kernel
+// adds the workers in index order.
+template <int MODEL, int R, bool MASK>
+__device__ __forceinline__ void sym_energy_chunk(const double (&a)[R], const double (&b)[R], const long long (&irow)[R],
+                                                 double2 q, long long jq, bool diag, double eps, double onepe,
+                                                 double (&acc)[R], double (&prod)[R], int (&esum)[R]) {
+    const unsigned lane = threadIdx.x & 31u, src = (lane + 31u) & 31u;
+#pragma unroll 4
+    for (int s = 0; s < 32; ++s) {
+        const double qnx = __shfl_sync(0xffffffffu, q.x, src);
+        const double qny = __shfl_sync(0xffffffffu, q.y, src);
+        const long long jqn = MASK ? __shfl_sync(0xffffffffu, jq, src) : 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            // counted: both particles exist, and inside the tile's own chunks only j > i
+            const bool on = !MASK || (irow[r] >= 0 && jq >= 0 && (!diag || jq > irow[r]));
+            if (MODEL == 1) {
+                const double d = fma(-b[r], q.y, fma(-a[r], q.x, onepe));
+                const double y = rsqrt_refined(d);
+                acc[r] += on ? y : 0.0;
+            } else {
+                const double dx = a[r] - q.x, dy = b[r] - q.y;
+                const double d = fma(dy, dy, fma(dx, dx, eps));
+                prod[r] *= on ? d : 1.0;
+            }
+        }
+        if (MODEL == 2 && (s & 7) == 7) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {   // move the exponent into the integer counter (2^-127 <= d <= 2^127)
+                const int hi = __double2hiint(prod[r]);
+                esum[r] += ((hi >> 20) & 0x7ff) - 1023;
+                prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
+            }
+        }
+        q.x = qnx;
+        q.y = qny;
+        if (MASK) jq = jqn;
+    }
+}
+
+template <int MODEL, int R>
+__global__ void __launch_bounds__(kSymThreads, 2)
+pair_energy_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, double pre, double* __restrict__ vpart) {
+    const int w = blockIdx.x * (kSymThreads / 32) + (threadIdx.x >> 5);
+    if (w >= S.G) return;
+    const int lane = threadIdx.x & 31;
+    const long long N = S.N;
+    const double onepe = 1.0 + eps;
+    constexpr double kLn2 = 0x1.62e42fefa39efp-1;
+    const int4 st = S.wstart[S.w0 + w];
+    int tile = st.x, chunk = st.y;
+    const bool ragged = (N % S.T) != 0 || (N % 32) != 0;
+
+    double a[R], b[R], acc[R], prod[R];
+    int esum[R];
+    long long irow[R];
+    double vsum = 0.0;
+    auto load_tile = [&](int t) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = (long long)t * S.T + r * 32 + lane;
+            irow[r] = i < N ? i : -1;
+            const double2 q = i < N ? js[i] : make_double2(0.0, 0.0);
+            a[r] = q.x;
+            b[r] = q.y;
+            acc[r] = 0.0;
+            prod[r] = 1.0;
+            esum[r] = 0;
+        }
+    };
+    auto close_tile = [&]() {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (MODEL == 2) acc[r] = fma((double)esum[r], kLn2, log(prod[r]));
+            vsum += acc[r];     // rows that do not exist never counted a pair: acc = 0 (Ring), log 1 = 0 (2D)
+        }
+    };
+    load_tile(tile);
+    long long jn = (long long)chunk * 32 + lane;
+    double2 qn = (jn < N) ? js[jn] : make_double2(0.0, 0.0);
+    for (int u = 0; u < st.z; ++u) {
+        const int ctile = tile, cchunk = chunk;
+        const long long j = jn;
+        const double2 q = qn;
+        ++chunk;
+        const bool tile_done = chunk == S.nchunks;
+        if (tile_done) { ++tile; chunk = tile * R; }
+        const bool more = u + 1 < st.z;
+        if (more) {
+            jn = (long long)chunk * 32 + lane;
+            qn = (jn < N) ? js[jn] : make_double2(0.0, 0.0);
+        }
+        const bool diag = cchunk < (ctile + 1) * R;
+        const bool masked = diag || (ragged && (ctile == S.ntiles - 1 || cchunk == S.nchunks - 1));
+        if (masked) sym_energy_chunk<MODEL, R, true>(a, b, irow, q, j < N ? j : -1, diag, eps, onepe, acc, prod, esum);
+        else sym_energy_chunk<MODEL, R, false>(a, b, irow, q, 0, false, eps, onepe, acc, prod, esum);
+        if (tile_done || !more) {
+            close_tile();
+            if (more) load_tile(tile);
+        }
+    }
+    vsum = warp_sum(vsum);
+    if (lane == 0) vpart[S.w0 + w] = pre * vsum;
+}
+
 // ---- update kernels (row a-U1) --------------------------------------------------------------------------
 
 constexpr int kUpdThreads = 256;

@@ -501,6 +501,27 @@ def test_symmetric_default_choice(lrmd, torch):
         x.close()
 
 
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N", [2, 33, 257, 1000, 4099, 10_007])
+def test_symmetric_energy_kernel_matches_oracle(lrmd, ref, torch, model, N):
+    """V from the symmetric walk (every unordered pair once, j > i inside a tile's own chunks), in one and in
+    several launches, both tile sizes."""
+    eps = _eps(model)
+    st = _state(model, N, 5000 + N)
+    q0, q1 = _q(model, st)
+    p0, p1 = _p(model, st)
+    e_ref, e_abs = ref.energy(model, eps, q0, q1, p0, p1)
+    for opts in ({lrmd.OPT_PAIR_VARIANT: 0}, {lrmd.OPT_PAIR_VARIANT: 1}, {lrmd.OPT_PAIR_SYM_TILES: 2, lrmd.OPT_PAIR_CTAS: 5}):
+        ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_SYMMETRIC: 1, **opts})
+        ctx.set_state(*st)
+        e = ctx.energy().cpu().numpy()
+        e2 = ctx.energy().cpu().numpy()
+        ctx.close()
+        assert abs(e[1] - e_ref[1]) <= 1e-12 * e_abs[1] + 1e-300, (opts, e[1], e_ref[1])
+        assert abs(e[0] - e_ref[0]) <= 1e-12 * e_abs[0] + 1e-300
+        assert np.array_equal(e, e2)
+
+
 # ---- fp32 pair arithmetic (SURVEY.md 8(f) N1; PAPER.md:110) -----------------------------------------
 
 F32TOL = 1e-5    # north_star: 1e-5 * sum_j |f_ij| for the fp32 variant
