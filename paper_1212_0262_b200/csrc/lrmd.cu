@@ -587,7 +587,7 @@ void pair_force_sym(Launcher& L) {
         }
         // rows of this batch only concern particles from its first tile on
         const long long first = (long long)S.tile0 * S.T;
-        L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N - first + 31) / 32)), dim3(32, 8), S, (const double*)i0,
+        L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N - first + 31) / 32)), dim3(32, kFoldGroups), S, (const double*)i0,
              (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
     }
 }

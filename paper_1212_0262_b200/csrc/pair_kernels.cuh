@@ -800,14 +800,17 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
 // Folds one launch (batch of tiles tile0 .. tile1 - 1) of the symmetric kernel into the force row out0 / out1:
 // for particle i (from the batch's first particle on) the i-side rows of the workers that touched i's tile, if the
 // tile is in the batch, + the j-side rows of the batch's tiles below i's tile.  The first batch writes, later ones
-// add (batches run in tile order on one stream).  Block = 32 particles x 8 row groups: group k adds the rows
-// k, k + 8, ... of each list in order, the 8 group sums are combined in a fixed tree: deterministic, and eight
-// times shorter than one dependent chain of ~100 loads per particle.
-__global__ void __launch_bounds__(256)
+// add (batches run in tile order on one stream).  Block = 32 particles x 16 row groups: group k adds the rows
+// k, k + 16, ... of each list in order, the group sums are combined in a fixed pairwise tree: deterministic, and
+// sixteen times shorter than one dependent chain of ~100 loads per particle.
+constexpr int kFoldGroups = 16;   // row groups per particle in pair_sym_fold_kernel (block = 32 x kFoldGroups threads)
+
+__global__ void __launch_bounds__(32 * kFoldGroups)
 pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
                      const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
                      double* __restrict__ out1) {
-    __shared__ double sf[8][32], sg[8][32];
+    constexpr int GR = kFoldGroups;
+    __shared__ double sf[GR][32], sg[GR][32];
     const long long N = S.N;
     const long long i = (long long)S.tile0 * S.T + (long long)blockIdx.x * 32 + threadIdx.x;
     const int k = threadIdx.y;
@@ -816,13 +819,13 @@ pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double*
         const int t = (int)(i / S.T);
         if (t < S.tile1) {
             const int2 rng = S.tile_rng[t];
-            for (int s = k; s <= rng.y - rng.x; s += 8) {
+            for (int s = k; s <= rng.y - rng.x; s += GR) {
                 f += ipart0[(long long)s * N + i];
                 if (ipart1) g += ipart1[(long long)s * N + i];
             }
         }
         const int nrows = (t < S.tile1 ? t : S.tile1) - S.tile0;     // batch tiles below i's tile
-        for (int a = k; a < nrows; a += 8) {
+        for (int a = k; a < nrows; a += GR) {
             f += jpart0[(long long)a * N + i];
             if (jpart1) g += jpart1[(long long)a * N + i];
         }
@@ -832,14 +835,20 @@ pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double*
     __syncthreads();
     if (k == 0 && i < N) {
         const int x = threadIdx.x;
-        const double ff = ((sf[0][x] + sf[1][x]) + (sf[2][x] + sf[3][x])) + ((sf[4][x] + sf[5][x]) + (sf[6][x] + sf[7][x]));
-        const double gg = ((sg[0][x] + sg[1][x]) + (sg[2][x] + sg[3][x])) + ((sg[4][x] + sg[5][x]) + (sg[6][x] + sg[7][x]));
+        double ff[GR], gg[GR];
+#pragma unroll
+        for (int m = 0; m < GR; ++m) { ff[m] = sf[m][x]; gg[m] = sg[m][x]; }
+#pragma unroll
+        for (int w = 1; w < GR; w *= 2) {      // fixed pairwise tree: (0+1), (2+3), ... then (01+23), ...
+#pragma unroll
+            for (int m = 0; m < GR; m += 2 * w) { ff[m] += ff[m + w]; gg[m] += gg[m + w]; }
+        }
         if (S.tile0 == 0) {
-            out0[i] = ff;
-            if (out1) out1[i] = gg;
+            out0[i] = ff[0];
+            if (out1) out1[i] = gg[0];
         } else {
-            out0[i] += ff;
-            if (out1) out1[i] += gg;
+            out0[i] += ff[0];
+            if (out1) out1[i] += gg[0];
         }
     }
 }
