@@ -158,10 +158,12 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     dev = torch.device("cuda", torch.cuda.current_device())
     peaks = measured_peaks()
     st = w.state()
-    ctx = lrmd.Context(w.model, w.N, w.eps, device=dev,
-                       options=({lrmd.OPT_PAIR_PRECISION: 1} if f32_pairs else
-                                ({lrmd.OPT_PAIR_SYMMETRIC: 0} if (ordered_pairs and w.model != 0) else
-                                 ({lrmd.OPT_PAIR_SYMMETRIC: 1} if force_symmetric else None))))
+    opts = {}
+    if f32_pairs:
+        opts[lrmd.OPT_PAIR_PRECISION] = 1
+    if w.model != 0 and (ordered_pairs or force_symmetric):
+        opts[lrmd.OPT_PAIR_SYMMETRIC] = 0 if ordered_pairs else 1
+    ctx = lrmd.Context(w.model, w.N, w.eps, device=dev, options=opts or None)
     ctx.set_state(*st)
     stream = torch.cuda.current_stream(dev)
     state_bytes = ctx.narrays * w.N * 8
@@ -254,13 +256,19 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                     "algorithmic_bytes_per_launch": bytes_per_launch}
         elif f32_pairs:
             # fp32 pair arithmetic: one MUFU.RCP per pair on the special-function unit, 16 lanes per SM per clock
-            mufu = float(w.N) * float(w.N)
+            sym = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
+            mufu = float(w.N) * float(w.N) * (0.5 if sym else 1.0)      # executed: one per (un)ordered pair evaluated
             peak = SM_COUNT * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
             achieved = mufu / avg_s / 1e12
-            roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T MUFU.RCP/s (= T pairs/s)",
+            roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T MUFU.RCP/s",
                     "frac": achieved / peak,
                     "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: 6 FADD/FFMA per pair",
                     "algorithmic_mufu_per_launch": mufu}
+            if sym:
+                roof["note"] = ("symmetric fp32 kernel: one MUFU.RCP and 8 FADD/FFMA per UNORDERED pair (N^2/2 evaluations deliver "
+                                "N^2 pair interactions), ~10.5 issued instructions per evaluation: instruction issue binds before "
+                                "the SFU; by the ordered-pair convention (one MUFU per delivered pair) the launch reads %.3f"
+                                % (float(w.N) * float(w.N) / avg_s / 1e12 / peak))
         else:
             sym = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
             flop = (SYM_PAIR_FLOP if sym else PAIR_FLOP)[w.model] * w.N * w.N
@@ -277,7 +285,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                                 "interactions); flops and instructions are the EXECUTED ones; by the ordered-pair convention "
                                 "(%g flop per delivered pair) the same launch reads %.3f of peak"
                                 % (PAIR_FLOP[w.model], PAIR_FLOP[w.model] * w.N * w.N / avg_s / 1e12 / peak))
-        roof.update({"kernel": {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel") if w.model == 0 else ("grav_force_f32_kernel" if f32_pairs else
+        roof.update({"kernel": {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel") if w.model == 0 else (("grav_force_sym_f32_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "grav_force_f32_kernel") if f32_pairs else
                                  ("pair_force_sym_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "pair_force_kernel")),
                      "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
                      "kernel_launches_per_force_evaluation": (kn / (3.0 * Kr)) if w.model != 0 else None,
@@ -472,6 +480,10 @@ def main():
                                                            "options", "clocks", "roofline") if k in r}
         others["grav2d_1m_f32pairs"]["steps"] = DEFAULT_STEPS["grav2d_1m"]
         others["grav2d_1m_f32pairs"]["dtype"] = "f32 pair terms, f64 state and accumulation"
+        r = run_workload(inputs.WORKLOADS["grav2d_1m"], 3, 3, None, with_e2e=False, f32_pairs=True, ordered_pairs=True)
+        others["grav2d_1m_f32pairs_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches",
+                                                                         "l2", "options", "clocks", "roofline") if k in r}
+        others["grav2d_1m_f32pairs_ordered_pairs"]["steps"] = 3
         line["others"] = others
         rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
         line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc}

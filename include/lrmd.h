@@ -79,7 +79,7 @@ enum {
     LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models, fp64: 1 = force kernel that evaluates every UNORDERED pair once and adds
                                     +f / -f to both particles (the paper declines this);
                                     0 = every ordered pair (the paper's scheme); -1 = choose (symmetric for N >= 2048
-                                    unless the context is a shard or uses fp32 pair terms).  With the symmetric
+                                    unless the context is a shard).  With the symmetric
                                     kernel LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, not CTAs.            */
     LRMD_OPT_PAIR_SYM_TILES = 9  /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
                                     N doubles per tile and component, within 1 GiB); get: the value in use            */

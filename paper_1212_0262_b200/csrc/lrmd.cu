@@ -126,7 +126,7 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     c->sym_tiles.clear();
     c->sym_batches.clear();
     const int64_t N = c->N;
-    if (c->opt_sym == 0 || c->N_total != c->N || c->opt_precision != 0) return;
+    if (c->opt_sym == 0 || c->N_total != c->N) return;
     if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
     // i per lane: Ring 4, 2D 8 (sweeps, profiles/); launch shape 0 / 1 asks for 4 / 8
     const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
@@ -578,7 +578,10 @@ void pair_force_sym(Launcher& L) {
         SymPart S = c->spart;
         S.tile0 = bt.x; S.tile1 = bt.y; S.w0 = bt.z; S.G = bt.w;
         const dim3 g((unsigned)((S.G + kSymThreads / 32 - 1) / (kSymThreads / 32))), b(kSymThreads);
-        if (c->model == LRMD_RING) {
+        if (c->opt_precision == 1) {
+            if (c->sym_R == 8) L.go_timed(grav_force_sym_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), S, (float)c->eps, pre, i0, i1, j0, j1);
+            else L.go_timed(grav_force_sym_f32_kernel<4>, g, b, (const float2*)js32_ptr(c), S, (float)c->eps, pre, i0, i1, j0, j1);
+        } else if (c->model == LRMD_RING) {
             if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<1, 8>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
             else L.go_timed(pair_force_sym_kernel<1, 4>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
         } else {

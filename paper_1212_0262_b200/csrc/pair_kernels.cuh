@@ -667,6 +667,128 @@ pair_energy_kernel(const double2* __restrict__ js, PairPart P, double eps, doubl
     if (threadIdx.x == 0) vpart[blockIdx.x] = pre_half * v[0];
 }
 
+// ---- symmetric force kernel, fp32 pair terms (rows N1 + N4) ---------------------------------------------------------
+// The same walk on the float2 position stream.  Halving the evaluations halves the MUFU.RCP count, the
+// unit that bounds grav_force_f32_kernel.  Precision follows reading G16: a lane's i-side sums run in fp32 over the 32
+// steps of one pass (32 terms) and are then added to its fp64 accumulators; the travelling j-side sum is fp64, fed
+// once per step with the fp32 sum of that step's R terms.
+template <int R, bool MASK, bool DIAG>
+__device__ __forceinline__ void sym_chunk_f32(const float (&a)[R], const float (&b)[R], const bool (&vi)[R],
+                                              double (&f0)[R], double (&f1)[R], float2 q, bool vq, float eps,
+                                              double& g0, double& g1) {
+    const unsigned lane = threadIdx.x & 31u, src = (lane + 31u) & 31u;
+    float sx[R], sy[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) sx[r] = sy[r] = 0.f;
+#pragma unroll 4
+    for (int s = 0; s < 32; ++s) {
+        const float qnx = __shfl_sync(0xffffffffu, q.x, src);
+        const float qny = __shfl_sync(0xffffffffu, q.y, src);
+        const bool vqn = MASK ? (__shfl_sync(0xffffffffu, (int)vq, src) != 0) : true;
+        float h0 = 0.f, h1 = 0.f;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float dx = a[r] - q.x, dy = b[r] - q.y;
+            const float r2 = fmaf(dy, dy, fmaf(dx, dx, eps));
+            float w = rcp_f32(r2);
+            if (MASK) w = (vi[r] && vq) ? w : 0.f;
+            sx[r] = fmaf(dx, w, sx[r]);
+            sy[r] = fmaf(dy, w, sy[r]);
+            if (!DIAG) {
+                h0 = fmaf(-dx, w, h0);
+                h1 = fmaf(-dy, w, h1);
+            }
+        }
+        if (!DIAG) {
+            g0 = __shfl_sync(0xffffffffu, g0 + (double)h0, src);
+            g1 = __shfl_sync(0xffffffffu, g1 + (double)h1, src);
+        }
+        q.x = qnx;
+        q.y = qny;
+        if (MASK) vq = vqn;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        f0[r] += (double)sx[r];
+        f1[r] += (double)sy[r];
+    }
+}
+
+template <int R>
+__global__ void __launch_bounds__(kSymThreads, 2)
+grav_force_sym_f32_kernel(const float2* __restrict__ js32, SymPart S, float eps, double pre, double* __restrict__ ipart0,
+                          double* __restrict__ ipart1, double* __restrict__ jpart0, double* __restrict__ jpart1) {
+    const int w = blockIdx.x * (kSymThreads / 32) + (threadIdx.x >> 5);
+    if (w >= S.G) return;
+    const int lane = threadIdx.x & 31;
+    const long long N = S.N;
+    const int4 st = S.wstart[S.w0 + w];
+    int tile = st.x, chunk = st.y;
+    const bool ragged = (N % S.T) != 0 || (N % 32) != 0;
+
+    float a[R], b[R];
+    double f0[R], f1[R];
+    bool vi[R];
+    auto load_tile = [&](int t) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = (long long)t * S.T + r * 32 + lane;
+            vi[r] = i < N;
+            const float2 q = vi[r] ? js32[i] : make_float2(0.f, 0.f);
+            a[r] = q.x;
+            b[r] = q.y;
+            f0[r] = 0.0;
+            f1[r] = 0.0;
+        }
+    };
+    auto store_tile = [&](int t) {
+        const int slot = S.w0 + w - S.tile_rng[t].x;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = (long long)t * S.T + r * 32 + lane;
+            if (vi[r]) {
+                ipart0[(long long)slot * N + i] = pre * f0[r];
+                ipart1[(long long)slot * N + i] = pre * f1[r];
+            }
+        }
+    };
+    load_tile(tile);
+    long long jn = (long long)chunk * 32 + lane;
+    float2 qn = (jn < N) ? js32[jn] : make_float2(0.f, 0.f);
+    for (int u = 0; u < st.z; ++u) {
+        const int ctile = tile, cchunk = chunk;
+        const long long j = jn;
+        const float2 q = qn;
+        const bool vq = j < N;
+        ++chunk;
+        const bool tile_done = chunk == S.nchunks;
+        if (tile_done) { ++tile; chunk = tile * R; }
+        const bool more = u + 1 < st.z;
+        if (more) {
+            jn = (long long)chunk * 32 + lane;
+            qn = (jn < N) ? js32[jn] : make_float2(0.f, 0.f);
+        }
+        double g0 = 0.0, g1 = 0.0;
+        const bool diag = cchunk < (ctile + 1) * R;
+        const bool masked = ragged && (ctile == S.ntiles - 1 || cchunk == S.nchunks - 1);
+        if (diag) {
+            if (masked) sym_chunk_f32<R, true, true>(a, b, vi, f0, f1, q, vq, eps, g0, g1);
+            else sym_chunk_f32<R, false, true>(a, b, vi, f0, f1, q, vq, eps, g0, g1);
+        } else {
+            if (masked) sym_chunk_f32<R, true, false>(a, b, vi, f0, f1, q, vq, eps, g0, g1);
+            else sym_chunk_f32<R, false, false>(a, b, vi, f0, f1, q, vq, eps, g0, g1);
+            if (vq) {
+                jpart0[(long long)(ctile - S.tile0) * N + j] = pre * g0;
+                jpart1[(long long)(ctile - S.tile0) * N + j] = pre * g1;
+            }
+        }
+        if (tile_done || !more) {
+            store_tile(ctile);
+            if (more) load_tile(tile);
+        }
+    }
+}
+
 // ---- symmetric potential-energy kernel -------------------------------------------------------------------------
 // V is a sum over unordered pairs to begin with (eqs.(1),(3): sum_{i<j}), so the walk of the symmetric force kernel
 // gives it with every pair evaluated once and nothing to send back: only the packet's position travels.  The chunks

@@ -534,12 +534,15 @@ def test_f32_pair_variant_forces(lrmd, ref, torch, N, variant):
     fp64 oracle; odd j-range boundaries exercise the 16-byte alignment of the fp32 tile copies."""
     st = _state(GRAV2D, N, 900 + N % 13)
     f0, f1, A0, A1 = ref.forces_abs(GRAV2D, 1e-3, st[0], st[1], form=0)
-    for ctas in (0, 7):
-        got = _gpu_forces(lrmd, GRAV2D, 1e-3, st, options={lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_VARIANT: variant,
-                                                          lrmd.OPT_PAIR_CTAS: ctas})
-        for g, w, a in ((got[0], f0, A0), (got[1], f1, A1)):
-            err = np.abs(g - w)
-            assert np.all(err <= F32TOL * a + 1e-300), float((err / np.maximum(a, 1e-300)).max())
+    for sym in (0, 1):          # every ordered pair (PAPER.md:110 as is) / every unordered pair once (N1 + N4)
+        for ctas in (0, 7):
+            if sym and variant == 2:
+                continue
+            got = _gpu_forces(lrmd, GRAV2D, 1e-3, st, options={lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_VARIANT: variant,
+                                                              lrmd.OPT_PAIR_CTAS: ctas, lrmd.OPT_PAIR_SYMMETRIC: sym})
+            for g, w, a in ((got[0], f0, A0), (got[1], f1, A1)):
+                err = np.abs(g - w)
+                assert np.all(err <= F32TOL * a + 1e-300), (sym, float((err / np.maximum(a, 1e-300)).max()))
 
 
 def test_f32_pair_variant_is_not_the_fp64_path_and_is_reproducible(lrmd, ref, torch):
