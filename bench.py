@@ -56,7 +56,7 @@ HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 NCU_TRAFFIC_BYTES = {"ring_16k": 279808.0, "grav2d_64k": 1067264.0, "hmf_5e7": 1541759232.0, "grav2d_1m": None,
                      "hmf_1e4": None, "grav2d_64k_f32": 554240.0,
                      # symmetric kernel (profiles/r01f_summary.md): j-stream reads + the j-side rows it writes
-                     "ring_16k_sym": 404480.0, "grav2d_64k_sym": 98298368.0}
+                     "ring_16k_sym": 404480.0, "grav2d_64k_sym": 98298368.0, "grav2d_64k_f32_sym": 95257600.0}
 
 DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5}
 
@@ -291,7 +291,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                      "kernel_launches_per_force_evaluation": (kn / (3.0 * Kr)) if w.model != 0 else None,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
                      "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else "") +
-                                                      ("_sym" if (w.model != 0 and not f32_pairs and
+                                                      ("_sym" if (w.model != 0 and
                                                                   ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1) else ""))})
         out["roofline"] = roof
 
