@@ -315,7 +315,7 @@ hmf_substage_tma_kernel(double* __restrict__ theta, double* __restrict__ p, long
 // particle-substage instead of two).  Deterministic: fixed particle -> thread map, fixed trees.
 constexpr int kHmfClusterCtas = 8;      // portable cluster size
 constexpr int kHmfClusterCtasMax = 16;  // non-portable size, used when the device grants it
-constexpr int kHmfClusterThreads = 640;
+constexpr int kHmfClusterThreads = 320;
 
 __device__ __forceinline__ unsigned cluster_ctarank() {
     unsigned r;

@@ -98,7 +98,7 @@ namespace {
 struct HmfVariant { int consumers, stages, minb; };
 constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}, {-1, 0, 0}};
 constexpr int kHmfClusterVariant = 3;   // cluster-resident kernel: whole state in registers, all steps in one launch
-constexpr int64_t kHmfClusterMaxN = (int64_t)kHmfClusterCtas * kHmfClusterThreads * 4;   // 20,480
+constexpr int64_t kHmfClusterMaxN = (int64_t)kHmfClusterCtas * kHmfClusterThreads * 8;   // 20,480
 constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
 constexpr int64_t kHmfTmaMinN = 1000000;
 constexpr double kSymRowBytes = 1073741824.0;   // scratch for the symmetric kernel's j-side rows per launch (1 GiB)
@@ -472,9 +472,9 @@ int hmf_step_cluster(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     const Coef k = coefficients();
     const int ctas = c->hmf_grid;     // 8, or 16 when the device grants the non-portable cluster size
     const int64_t per = (int64_t)ctas * kHmfClusterThreads;
-    const int P = c->N <= per ? 1 : (c->N <= 2 * per ? 2 : 4);
+    const int P = c->N <= per ? 1 : (c->N <= 2 * per ? 2 : (c->N <= 4 * per ? 4 : 8));
     void (*kernel)(double*, double*, long long, long long, double, double, double, double, double2*) =
-        P == 1 ? hmf_cluster_kernel<1> : (P == 2 ? hmf_cluster_kernel<2> : hmf_cluster_kernel<4>);
+        P == 1 ? hmf_cluster_kernel<1> : (P == 2 ? hmf_cluster_kernel<2> : (P == 4 ? hmf_cluster_kernel<4> : hmf_cluster_kernel<8>));
     if (ctas > kHmfClusterCtas) {
         bool ready = false;
         for (const void* f : c->smem_ready) ready = ready || f == (const void*)kernel;

@@ -131,9 +131,9 @@ def test_hmf_tma_variants_match_oracle(lrmd, ref, torch, variant, N):
     assert abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N) + 1e-300
 
 
-@pytest.mark.parametrize("N", [1, 2, 31, 640, 5119, 5120, 5121, 10_000, 10_241, 20_480])
+@pytest.mark.parametrize("N", [1, 2, 31, 640, 2559, 2560, 2561, 5121, 10_000, 10_241, 20_480])
 def test_hmf_cluster_resident_kernel_matches_oracle(lrmd, ref, torch, N):
-    """Cluster-resident HMF kernel (variant 3; 1, 2 or 4 particles per thread): 7-step trajectory, the
+    """Cluster-resident HMF kernel (variant 3; 1, 2, 4 or 8 particles per thread): 7-step trajectory, the
     cached sums it leaves behind (forces, energy) and step(n) == n x step(1) bit for bit."""
     st = _state(HMF, N, 300 + N % 11)
     ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: 3})
