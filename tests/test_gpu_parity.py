@@ -794,3 +794,40 @@ def test_paper_shaped_runs_conserve_energy(lrmd, torch):
         assert out["K"][0] == 0.0 and len(out["K"]) == 7
         assert out["K"][-1] > 0.0
         assert max(out["energy_error"]) < tol, (name, max(out["energy_error"]))
+
+
+# ---- option combinations ------------------------------------------------------------------------------------------
+
+def test_random_option_combinations_match_oracle(lrmd, ref, torch):
+    """60 seeded combinations of (model, N, kernel choice, launch shape, workers / CTAs, tiles per launch, pair
+    precision): forces within tolerance of the oracle and a 2-step trajectory within 1e-9 (1e-6 with fp32 pairs)."""
+    rng = np.random.default_rng(20121204)
+    for case in range(60):
+        model = int(rng.choice([RING, GRAV2D]))
+        N = int(rng.choice([1, 2, 31, 33, 200, 257, 1000, 2047, 2048, 2500, 4097]))
+        opts = {lrmd.OPT_PAIR_SYMMETRIC: int(rng.choice([-1, 0, 1])), lrmd.OPT_PAIR_VARIANT: int(rng.choice([-1, 0, 1, 2])),
+                lrmd.OPT_PAIR_CTAS: int(rng.choice([0, 1, 3, 40, 700])), lrmd.OPT_PAIR_SYM_TILES: int(rng.choice([0, 1, 5]))}
+        f32 = model == GRAV2D and rng.random() < 0.3
+        if f32:
+            opts[lrmd.OPT_PAIR_PRECISION] = 1
+        eps = _eps(model)
+        st = _state(model, N, 9000 + case)
+        q0, q1 = _q(model, st)
+        f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+        ctx = lrmd.Context(model, N, eps, options=opts)
+        ctx.set_state(*st)
+        f = ctx.forces()
+        got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+        ftol = F32TOL if f32 else FTOL
+        for g, w, a in zip(got, (f0, f1), (A0, A1)):
+            if g is not None:
+                assert np.all(np.abs(g - w) <= ftol * a + 1e-300), (case, model, N, opts)
+        ctx.step(2, 0.01)
+        out = ctx.state_numpy()
+        ctx.close()
+        r = [a.copy() for a in st]
+        rq0, rq1 = _q(model, r)
+        rp0, rp1 = _p(model, r)
+        ref.step(model, eps, rq0, rq1, rp0, rp1, 2, 0.01, form=1)
+        for g, w in zip(out, r):
+            assert np.max(np.abs(g - w)) <= (1e-6 if f32 else XTOL), (case, model, N, opts)
