@@ -81,8 +81,11 @@ enum {
                                     0 = every ordered pair (the paper's scheme); -1 = choose (symmetric for N >= 2048
                                     unless the context is a shard).  With the symmetric
                                     kernel LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, not CTAs.            */
-    LRMD_OPT_PAIR_SYM_TILES = 9  /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
+    LRMD_OPT_PAIR_SYM_TILES = 9, /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
                                     N doubles per tile and component, within 1 GiB); get: the value in use            */
+    LRMD_OPT_PAIR_FUSE_UPDATE = 10 /* symmetric kernel, one launch per force evaluation: 0 = separate update kernel,
+                                    1 / -1 = the kick / drift that follows a force evaluation runs inside its fold
+                                    kernel (same arithmetic, bit-identical results); get: whether it is in use       */
 };
 
 /* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.

@@ -53,7 +53,7 @@ struct lrmd_ctx {
     void* coll_user = nullptr;
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
-    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0;
+    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0, opt_fuse = -1;
     // resolved
     int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
     int slots = 1;              // partial force rows per particle (pair models)
@@ -570,7 +570,9 @@ void pair_pack(Launcher& L) {
 inline double* wsd(lrmd_ctx* c, size_t off) { return off ? reinterpret_cast<double*>(c->ws + off) : nullptr; }
 
 // Symmetric force evaluation (row N4): per batch of tiles one kernel launch + the fold into the force row.
-void pair_force_sym(Launcher& L) {
+// upd: 0 = none, 1 kick, 2 kick + drift, 3 two kicks + drift, fused into the fold (single-launch evaluations only;
+// the caller checks pair_can_fuse).
+void pair_force_sym(Launcher& L, int upd = 0, double kickA = 0.0, double kickB = 0.0, double drift = 0.0) {
     lrmd_ctx* c = L.c;
     double *i0 = wsd(c, c->lay.ipart0), *i1 = wsd(c, c->lay.ipart1), *j0 = wsd(c, c->lay.jpart0), *j1 = wsd(c, c->lay.jpart1);
     const double pre = c->model == LRMD_RING ? -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N) : -2.0 / (double)c->N;
@@ -590,8 +592,20 @@ void pair_force_sym(Launcher& L) {
         }
         // rows of this batch only concern particles from its first tile on
         const long long first = (long long)S.tile0 * S.T;
-        L.go(pair_sym_fold_kernel, dim3((unsigned)((c->N - first + 31) / 32)), dim3(32, kFoldGroups), S, (const double*)i0,
-             (const double*)i1, (const double*)j0, (const double*)j1, part0(c), part1(c));
+        FusedUpdate U;
+        U.q0 = c->a0; U.q1 = nullptr; U.p0 = c->a1; U.p1 = nullptr;
+        if (c->model == LRMD_GRAV2D) { U.q1 = c->a1; U.p0 = c->a2; U.p1 = c->a3; }
+        U.kickA = kickA; U.kickB = kickB; U.drift = drift; U.js = js_ptr(c); U.js32 = js32_ptr(c);
+        const dim3 fg((unsigned)((c->N - first + 31) / 32)), fb(32, kFoldGroups);
+#define LRMD_FOLD(M, UPD) \
+        L.go(pair_sym_fold_kernel<M, UPD>, fg, fb, S, (const double*)i0, (const double*)i1, (const double*)j0, \
+             (const double*)j1, part0(c), part1(c), U)
+        if (c->model == LRMD_RING) {
+            if (upd == 1) LRMD_FOLD(1, 1); else if (upd == 2) LRMD_FOLD(1, 2); else if (upd == 3) LRMD_FOLD(1, 3); else LRMD_FOLD(1, 0);
+        } else {
+            if (upd == 1) LRMD_FOLD(2, 1); else if (upd == 2) LRMD_FOLD(2, 2); else if (upd == 3) LRMD_FOLD(2, 3); else LRMD_FOLD(2, 0);
+        }
+#undef LRMD_FOLD
     }
 }
 
@@ -651,15 +665,24 @@ int pair_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     const Coef k = coefficients();
     Launcher L{c, stream};
     pair_ensure_force(L);
+    // A force evaluation that is one launch of the symmetric kernel takes the update that follows it into its
+    // fold kernel (same arithmetic, one launch and one pass over the force row fewer per substage).
+    const bool fuse = c->sym && c->sym_batches.size() == 1 && c->opt_fuse != 0;
+    auto force_then_update = [&](bool kick2, bool drift, double kA, double kB, double d) {
+        if (fuse) {
+            pair_force_sym(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
+        } else {
+            pair_force(L);
+            pair_update(L, kick2, drift, kA, kB, d);
+        }
+    };
+    pair_update(L, false, true, k.B0 * dt, 0.0, k.D0 * dt);
     for (int64_t s = 0; s < n; ++s) {
-        pair_update(L, s > 0, true, k.B0 * dt, k.B0 * dt, k.D0 * dt);
-        pair_force(L);
-        pair_update(L, false, true, k.B1 * dt, 0.0, k.D1 * dt);
-        pair_force(L);
-        pair_update(L, false, true, k.B1 * dt, 0.0, k.D0 * dt);
-        pair_force(L);
+        force_then_update(false, true, k.B1 * dt, 0.0, k.D1 * dt);
+        force_then_update(false, true, k.B1 * dt, 0.0, k.D0 * dt);
+        if (s + 1 < n) force_then_update(true, true, k.B0 * dt, k.B0 * dt, k.D0 * dt);   // closing + opening kick
+        else force_then_update(false, false, k.B0 * dt, 0.0, 0.0);                       // closing kick
     }
-    pair_update(L, false, false, k.B0 * dt, 0.0, 0.0);
     return L.rc;
 }
 
@@ -936,6 +959,10 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
             c->opt_sym = value;
             break;
+        case LRMD_OPT_PAIR_FUSE_UPDATE:
+            if (value < -1 || value > 1) return LRMD_EINVAL;
+            c->opt_fuse = value;
+            return LRMD_OK;
         case LRMD_OPT_PAIR_SYM_TILES:
             if (value < 0 || value > (1 << 24)) return LRMD_EINVAL;
             if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
@@ -968,6 +995,7 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
         case LRMD_OPT_PAIR_SLOTS: *value = c->sym ? c->sym_slots : c->slots; break;
         case LRMD_OPT_PAIR_SYMMETRIC: *value = c->sym ? 1 : 0; break;
         case LRMD_OPT_PAIR_SYM_TILES: *value = c->sym ? c->sym_rows : 0; break;
+        case LRMD_OPT_PAIR_FUSE_UPDATE: *value = (c->sym && c->sym_batches.size() == 1 && c->opt_fuse != 0) ? 1 : 0; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;

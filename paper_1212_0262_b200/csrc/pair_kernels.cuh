@@ -927,10 +927,20 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
 // sixteen times shorter than one dependent chain of ~100 loads per particle.
 constexpr int kFoldGroups = 16;   // row groups per particle in pair_sym_fold_kernel (block = 32 x kFoldGroups threads)
 
+// The update that follows a force evaluation (pair_update_kernel's arithmetic), fused into the fold of a
+// single-launch evaluation: UPD = 0 none, 1 kick, 2 kick + drift, 3 two kicks + drift.
+struct FusedUpdate {
+    double *q0, *q1, *p0, *p1;
+    double kickA, kickB, drift;
+    double2* js;
+    float2* js32;
+};
+
+template <int MODEL, int UPD>
 __global__ void __launch_bounds__(32 * kFoldGroups)
 pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
                      const double* __restrict__ jpart0, const double* __restrict__ jpart1, double* __restrict__ out0,
-                     double* __restrict__ out1) {
+                     double* __restrict__ out1, FusedUpdate U) {
     constexpr int GR = kFoldGroups;
     __shared__ double sf[GR][32], sg[GR][32];
     const long long N = S.N;
@@ -971,6 +981,31 @@ pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double*
         } else {
             out0[i] += ff[0];
             if (out1) out1[i] += gg[0];
+        }
+        if (UPD != 0) {     // only on single-launch evaluations (tile0 = 0, tile1 = ntiles): ff, gg are the force
+            double p = fma(U.kickA, ff[0], U.p0[i]);
+            if (UPD == 3) p = fma(U.kickB, ff[0], p);
+            U.p0[i] = p;
+            double pb = 0.0;
+            if (MODEL == 2) {
+                pb = fma(U.kickA, gg[0], U.p1[i]);
+                if (UPD == 3) pb = fma(U.kickB, gg[0], pb);
+                U.p1[i] = pb;
+            }
+            if (UPD >= 2) {
+                const double x = fma(U.drift, p, U.q0[i]);
+                U.q0[i] = x;
+                if (MODEL == 2) {
+                    const double y = fma(U.drift, pb, U.q1[i]);
+                    U.q1[i] = y;
+                    U.js[i] = make_double2(x, y);
+                    if (U.js32) U.js32[i] = make_float2((float)x, (float)y);
+                } else {
+                    double sn, cs;
+                    sincos_any(x, sn, cs);
+                    U.js[i] = make_double2(cs, sn);
+                }
+            }
         }
     }
 }

@@ -796,6 +796,33 @@ def test_paper_shaped_runs_conserve_energy(lrmd, torch):
         assert max(out["energy_error"]) < tol, (name, max(out["energy_error"]))
 
 
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+def test_update_fused_into_fold_is_bit_identical(lrmd, torch, model):
+    """LRMD_OPT_PAIR_FUSE_UPDATE: the kick / drift after a single-launch symmetric force evaluation runs inside the
+    fold kernel; same arithmetic, so trajectories, cached forces and energies are bit-identical to the separate
+    update kernel, for step(n) and for n x step(1)."""
+    eps = _eps(model)
+    N = 5003
+    st = _state(model, N, 321)
+    res = []
+    for fuse, single in ((1, False), (0, False), (1, True)):
+        ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_FUSE_UPDATE: fuse})
+        assert ctx.get_option(lrmd.OPT_PAIR_FUSE_UPDATE) == fuse
+        ctx.set_state(*st)
+        if single:
+            for _ in range(6):
+                ctx.step(1, 0.01)
+        else:
+            ctx.step(6, 0.01)
+        f = ctx.forces()
+        f = [t.cpu().numpy() for t in f] if model == GRAV2D else [f.cpu().numpy()]
+        res.append(list(ctx.state_numpy()) + f + [ctx.energy().cpu().numpy()])
+        ctx.close()
+    for other in res[1:]:
+        for x, y in zip(res[0], other):
+            assert np.array_equal(x, y)
+
+
 # ---- option combinations ------------------------------------------------------------------------------------------
 
 def test_random_option_combinations_match_oracle(lrmd, ref, torch):
