@@ -1,19 +1,26 @@
 #!/usr/bin/env python
 """bench.py — throughput of the lrmd hot path on B200, one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload KEY] [--only] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload KEY] [--only] [--f32-pairs] [--impl reference]
 
 A bench "step" is one complete integrator time step of the workload (three force
 evaluations + the kick/drift updates — what the paper's Tables 1-3 time).  The primary workload is
 BASELINE.json configs[1] (Ring, N = 16,384, eps = 0.01, dt = 0.01); with one GPU and without --only
-the other single-GPU configs are measured too and reported under "others" in the same line.
+the other single-GPU configs are measured too and reported under "others" in the same line, together
+with the ordered-pair kernels (the paper's own scheme, LRMD_OPT_PAIR_SYMMETRIC = 0) on the pair configs
+and config 5's fp32-pair variant.
 
 Numbers reported (all measured in this process, never under a profiler):
   value      whole-job throughput, state resident in HBM, CUDA events on the launching stream
   e2e        the same metric through lrmd_step_host: pinned HOST buffers, H2D + (3K+1) force
              evaluations + D2H inside the timed region
-  roofline   the dominant kernel (pair-force kernel / HMF fused substage): algorithmic flops or bytes
-             per launch / its average launch duration (event pairs around every launch, second pass)
+  roofline   the dominant kernel (pair-force kernel / HMF fused substage): work per force evaluation (pair
+             models) or per launch (HMF) / its device time from event pairs around every launch (second pass).
+             Pair models: EXECUTED flops against 148 x 64 x 2 x f_max; the symmetric kernel evaluates every
+             unordered pair once, so its executed work per delivered pair is about half the ordered kernels'
+             (roofline.note gives the ordered-pair-convention figure as well).  HMF: 32 B per particle-substage
+             against the measured HBM copy bandwidth.
+  energy     lrmd_energy timed apart from the steps
   cpu_baseline  the oracle (oracle/lrmd_ref.cpp), as it stands, on this box's host cores, bounded sample
 
 Multi-GPU (torchrun, --gpus N): the path does not shard under BASELINE.json's north_star ("no sharding
