@@ -141,8 +141,21 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     if (TB < 1) TB = 1;
     if (TB > ntiles) TB = ntiles;
     // workers per launch: 32 per SM (4 waves of the 8 resident warps; sweeps in profiles/); at least two units each
-    const int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas
-                          : (int64_t)kNumSm * 32;
+    int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * 32;
+    // the host-built work table has one entry per worker and launch: keep it below 2^22 entries (64 MB)
+    const int64_t nbatches = (ntiles + TB - 1) / TB;
+    if (c->opt_pair_ctas <= 0) {
+        // a tile's i-side rows number about workers / tiles per launch: keep them within ~4 GiB
+        int64_t maxslots = (int64_t)(4.0 * 1073741824.0 / ((double)N * 8.0 * comps));
+        if (maxslots < 8) maxslots = 8;
+        if (Gwant > maxslots * TB) Gwant = maxslots * TB;
+        if (Gwant < (int64_t)kNumSm * 8) Gwant = (int64_t)kNumSm * 8;
+    }
+    if (c->opt_pair_ctas <= 0 && nbatches * Gwant > ((int64_t)1 << 22)) {
+        Gwant = ((int64_t)1 << 22) / nbatches;
+        if (Gwant < (int64_t)kNumSm * 8) return;    // launches would not fill the GPU (N beyond ~8e6): ordered kernel
+    }
+    if (nbatches * Gwant > ((int64_t)1 << 26)) return;
     c->sym_tiles.assign((size_t)ntiles, make_int2(0x7fffffff, -1));
     int gmax = 1;
     for (int64_t t0 = 0; t0 < ntiles; t0 += TB) {
