@@ -858,3 +858,31 @@ def test_random_option_combinations_match_oracle(lrmd, ref, torch):
         ref.step(model, eps, rq0, rq1, rp0, rp1, 2, 0.01, form=1)
         for g, w in zip(out, r):
             assert np.max(np.abs(g - w)) <= (1e-6 if f32 else XTOL), (case, model, N, opts)
+
+
+def test_random_hmf_option_combinations_match_oracle(lrmd, ref, torch):
+    """40 seeded combinations of (N, kernel variant, grid, graph replay): forces at the final angles, a 9-step
+    trajectory (graph replay needs >= 8 steady-state steps) and the energies against the oracle."""
+    rng = np.random.default_rng(20121205)
+    for case in range(40):
+        N = int(rng.choice([1, 3, 4, 1000, 2049, 20_480, 20_481, 65_537, 300_000]))
+        opts = {lrmd.OPT_HMF_VARIANT: int(rng.choice([-1, 0, 1, 2, 3])), lrmd.OPT_GRAPH: int(rng.choice([-1, 0, 1])),
+                lrmd.OPT_HMF_GRID: int(rng.choice([0, 0, 1, 7, 148]))}
+        if opts[lrmd.OPT_HMF_VARIANT] == 3 and opts[lrmd.OPT_HMF_GRID] not in (0,):
+            opts[lrmd.OPT_HMF_GRID] = 0          # the cluster-resident kernel takes 0 (8 CTAs) or 16 only
+        st = _state(HMF, N, 7000 + case)
+        ctx = lrmd.Context(HMF, N, 0.0, options=opts)
+        ctx.set_state(*st)
+        ctx.step(9, 0.05)
+        out = ctx.state_numpy()
+        f = ctx.forces().cpu().numpy()
+        e = ctx.energy().cpu().numpy()
+        ctx.close()
+        th, p = st[0].copy(), st[1].copy()
+        ref.step(HMF, 0.0, th, None, p, None, 9, 0.05, form=0)
+        assert np.max(np.abs(out[0] - th)) <= XTOL and np.max(np.abs(out[1] - p)) <= XTOL, (case, N, opts)
+        f0, _, S0, _ = ref.forces_abs(HMF, 0.0, out[0], None, form=0)
+        assert np.all(np.abs(f - f0) <= FTOL * S0 + 4e-16), (case, N, opts)
+        er, ea = ref.energy(HMF, 0.0, out[0], None, out[1], None)
+        assert abs(e[0] - er[0]) <= 1e-12 * ea[0] + 1e-300, (case, N, opts)
+        assert abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N) + 1e-300, (case, N, opts)
