@@ -390,7 +390,7 @@ __device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b
                                           double (&f0)[R], double (&f1)[R], double2 q, bool vq, double eps,
                                           double onepe, double& g0, double& g1) {
     const unsigned lane = threadIdx.x & 31u, src = (lane + 31u) & 31u;   // the packet moves to lane + 1
-#pragma unroll 4
+#pragma unroll 8
     for (int s = 0; s < 32; ++s) {
         // the position part of the next packet is requested before this step's arithmetic; the force part
         // is summed per step (h0, h1) and joins the travelling sum only at the end, so that the shuffle
