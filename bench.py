@@ -413,6 +413,45 @@ def run_reference(args, w):
     return 0
 
 
+def fp64_peak_table(device=None, iters=20000, full=True):
+    """bench.py --fp64-peak: the committed FP64 issue-rate microbenchmark (lrmd_fp64_peak), one JSON object.
+    `peak` = the best sustained DFMA rate over the resident-warp sweep; `mixes` = FP64 lanes busy per clock per SM
+    when each group of 16 DFMA carries k instructions of another class (what a non-FP64 instruction costs)."""
+    import torch
+    from paper_1212_0262_b200 import lrmd
+    dev = device or torch.device("cuda", torch.cuda.current_device())
+    scratch = torch.empty(148 * 64 * 32 * 8 + 148 * 64 * 4 + 4096 + 256, dtype=torch.uint8, device=dev)
+    ptr = (scratch.data_ptr() + 255) // 256 * 256
+    stream = int(torch.cuda.current_stream(dev).cuda_stream)
+
+    def run(op, mix, xn, warps):
+        rc, out = lrmd.lrmd_fp64_peak(op, mix, xn, warps, iters, ptr, scratch.numel() - 256, stream)
+        if rc != lrmd.OK:
+            raise lrmd.LrmdError(rc, "lrmd_fp64_peak")
+        return {"instr_per_s": out[0], "sm_mhz": out[1], "lanes_per_clk_per_sm": out[2], "ms": out[3]}
+
+    res = {"what": "lrmd_fp64_peak: 16 independent FP64 chains per thread, 148 x warps_per_sm warps, CUDA events around one launch; "
+                   "sm_mhz = clock64 / globaltimer inside the kernel", "iters": iters, "ops": {}, "mixes": {}}
+    best = None
+    for name, op in (("dfma", 0), ("dmul", 1), ("dadd", 2), ("dfma_3_private_regs", 3), ("dfma_1_shared_reg", 4),
+                     ("dfma_square", 5), ("dfma_imm_addend", 6)):
+        res["ops"][name] = {}
+        for warps in ((4, 8, 16, 32, 64) if full else (32,)):
+            r = run(op, 0, 0, warps)
+            res["ops"][name][str(warps)] = r
+            if op == 0 and (best is None or r["instr_per_s"] > best["instr_per_s"]):
+                best = dict(r, warps_per_sm=warps)
+    res["peak"] = best
+    if full:
+        for name, mix in (("int_lop3", 1), ("mufu_rcp64h", 2), ("shfl", 3), ("lds64", 4), ("mufu_seed_plus_dfma", 5),
+                          ("mov", 6), ("sts64", 7)):
+            res["mixes"][name] = {}
+            for warps in (8, 16, 32):
+                res["mixes"][name][str(warps)] = {str(xn): run(0, mix, xn, warps)["lanes_per_clk_per_sm"] for xn in (2, 4, 8, 16)}
+    del scratch
+    return res
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -423,7 +462,17 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--f32-pairs", action="store_true", help="GRAV2D workloads: fp32 pair arithmetic (PAPER.md:110)")
+    ap.add_argument("--fp64-peak", action="store_true", help="run only the FP64 issue-rate microbenchmark and print its table")
     args = ap.parse_args()
+
+    if args.fp64_peak:
+        import torch
+        from paper_1212_0262_b200 import lrmd
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+        lrmd.load()
+        print(json.dumps(fp64_peak_table()))
+        return 0
 
     from paper_1212_0262_b200 import inputs
     w = inputs.WORKLOADS[args.workload]

@@ -187,6 +187,21 @@ int lrmd_coefficients(double* out4_host);
  * so that its accuracy can be checked against a multiprecision reference without a GPU. */
 int lrmd_host_sincos(const double* x_host, int64_t n, double* s_host, double* c_host);
 
+/* Diagnostic (measurement aid, not on the hot path; SYNCHRONISES the stream): FP64 issue-rate microbenchmark, the
+ * measured counterpart of the derived `alu` roofline denominator 148 SMs x 64 FP64 lanes x clock that bounds the
+ * pair kernels (SURVEY.md section 7 hard part 8).  Every thread of 148 x warps_per_sm warps
+ * (warps_per_sm a multiple of 4, 4..64) runs `iters` rounds of 16 independent chains of op (0 = DFMA with two
+ * operands shared by all chains, 1 = DMUL, 2 = DADD, 3 = DFMA on three private registers, 4 = DFMA with one shared
+ * operand, 5 = DFMA a*a+c, 6 = DFMA with an immediate addend) and, per round, extra_per_16 (0, 2, 4, 8 or 16)
+ * instructions of class mix (0 none, 1 integer LOP3, 2 MUFU.RCP64H, 3 SHFL, 4 LDS.64, 5 MUFU.RCP64H seed + the DFMA
+ * that consumes it, 6 MOV, 7 STS.64), op = 0 only for mix != 0.
+ * scratch_device: DEVICE, 256-byte aligned, at least 148 x warps_per_sm x 32 x 8 + 148 x warps_per_sm x 4 + 1024
+ * bytes, caller-owned.  out4_host (HOST) = {FP64 instructions per second (thread level), SM clock held in MHz
+ * (clock64 over globaltimer inside the kernel), FP64 lanes busy per clock per SM, kernel milliseconds}.
+ * Unknown combination: LRMD_EUNSUPPORTED.  Needs no context. */
+int lrmd_fp64_peak(int op, int mix, int extra_per_16, int warps_per_sm, int iters, void* scratch_device,
+                   size_t scratch_bytes, double* out4_host, void* cuda_stream);
+
 /* Diagnostic (HOST pointers, runs on the CPU, no GPU needed): the work partition of the pair kernels
  * (RING, GRAV2D) for the current options.  The N x N pair rectangle (every ordered pair is computed,
  * PAPER.md:108; tiles after PAPER.md:100-106) is cut into i-tiles; the flattened (i-tile, j) space is

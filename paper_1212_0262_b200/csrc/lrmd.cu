@@ -14,6 +14,7 @@
 
 #include "hmf_kernels.cuh"
 #include "pair_kernels.cuh"
+#include "peak_kernels.cuh"
 
 namespace {
 
@@ -1094,6 +1095,67 @@ int lrmd_pair_sym_partition(const lrmd_ctx* c, int64_t worker, int64_t* out5_hos
     out5_host[2] = st.z;                   // number of (tile, chunk) units, tile-major
     out5_host[3] = batch;                  // launch (batch of tiles) the worker belongs to
     out5_host[4] = 32 * c->sym_R;          // particles per i-tile
+    return LRMD_OK;
+}
+
+int lrmd_fp64_peak(int op, int mix, int extra_per_16, int warps_per_sm, int iters, void* scratch_device,
+                   size_t scratch_bytes, double* out4_host, void* cuda_stream) {
+    if (!scratch_device || !out4_host || iters < 1 || warps_per_sm < 4 || warps_per_sm > 64 || (warps_per_sm % 4) != 0)
+        return LRMD_EINVAL;
+    if (((uintptr_t)scratch_device % kAlign) != 0) return LRMD_EINVAL;
+    using Kern = void (*)(double*, const double*, int, unsigned long long*);
+    Kern kern = nullptr;
+#define LRMD_PEAK(OP, XK, XN) if (op == OP && mix == XK && extra_per_16 == XN) kern = fp64_peak_kernel<OP, XK, XN>
+    LRMD_PEAK(kPeakDfma, kMixNone, 0); LRMD_PEAK(kPeakDmul, kMixNone, 0); LRMD_PEAK(kPeakDadd, kMixNone, 0);
+    LRMD_PEAK(kPeakDfma3, kMixNone, 0); LRMD_PEAK(kPeakDfma2, kMixNone, 0); LRMD_PEAK(kPeakDfmaSq, kMixNone, 0);
+    LRMD_PEAK(kPeakDfmaImm, kMixNone, 0);
+#define LRMD_PEAK3(XK) LRMD_PEAK(kPeakDfma, XK, 2); LRMD_PEAK(kPeakDfma, XK, 4); LRMD_PEAK(kPeakDfma, XK, 8); LRMD_PEAK(kPeakDfma, XK, 16)
+    LRMD_PEAK3(kMixInt); LRMD_PEAK3(kMixMufu); LRMD_PEAK3(kMixShfl); LRMD_PEAK3(kMixLds); LRMD_PEAK3(kMixMufuSeed);
+    LRMD_PEAK3(kMixMov); LRMD_PEAK3(kMixSts);
+#undef LRMD_PEAK3
+#undef LRMD_PEAK
+    if (!kern) return LRMD_EUNSUPPORTED;
+    const int grid = kNumSm * (warps_per_sm / (kPeakThreads / 32));
+    const size_t out_bytes = align_up(sizeof(double) * (size_t)grid * kPeakThreads);
+    const size_t seed_bytes = align_up(sizeof(double) * 4);
+    const size_t clk_bytes = align_up(sizeof(unsigned long long) * 2 * (size_t)grid);
+    if (scratch_bytes < out_bytes + seed_bytes + clk_bytes) return LRMD_EINVAL;
+    char* base = static_cast<char*>(scratch_device);
+    double* out = reinterpret_cast<double*>(base);
+    double* seedv = reinterpret_cast<double*>(base + out_bytes);
+    unsigned long long* clk = reinterpret_cast<unsigned long long*>(base + out_bytes + seed_bytes);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    // operands of the chains: a <- a * m + c stays finite and normal for any number of iterations
+    const double seed[4] = {0.99999999, 1.0e-3, 1.0, 0.0};
+    std::vector<unsigned long long> hclk(2 * (size_t)grid);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaMemcpyAsync(seedv, seed, sizeof(seed), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        kern<<<grid, kPeakThreads, 0, st>>>(out, seedv, iters > 64 ? 64 : iters, clk);     // warm-up
+        cudaEventRecord(e0, st);
+        kern<<<grid, kPeakThreads, 0, st>>>(out, seedv, iters, clk);
+        cudaEventRecord(e1, st);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(hclk.data(), clk, sizeof(unsigned long long) * hclk.size(), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return LRMD_ECUDA; }
+    double cyc = 0.0, ns = 0.0;
+    for (int b = 0; b < grid; ++b) { cyc += (double)hclk[2 * b]; ns += (double)hclk[2 * b + 1]; }
+    const double fp64_per_thread = (double)iters * (kPeakChains + (mix == kMixMufuSeed ? extra_per_16 : 0));
+    const double instr = fp64_per_thread * (double)grid * kPeakThreads;     // thread-level FP64 instructions
+    const double mhz = ns > 0.0 ? cyc / ns * 1e3 : 0.0;
+    out4_host[0] = instr / ((double)ms * 1e-3);                               // FP64 instructions per second
+    out4_host[1] = mhz;                                                       // SM clock held (clock64 / globaltimer)
+    out4_host[2] = mhz > 0.0 ? out4_host[0] / (mhz * 1e6 * kNumSm) : 0.0;    // FP64 lanes busy per clock per SM
+    out4_host[3] = (double)ms;
     return LRMD_OK;
 }
 

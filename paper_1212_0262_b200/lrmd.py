@@ -26,7 +26,7 @@ SYMBOLS = (
     "lrmd_create", "lrmd_destroy", "lrmd_workspace_bytes", "lrmd_set_workspace", "lrmd_set_state",
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
-    "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard", "lrmd_pair_sym_partition",
+    "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard", "lrmd_pair_sym_partition", "lrmd_fp64_peak",
 )
 
 _lib = None
@@ -80,6 +80,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_step_observe.argtypes = [_vp, _i64, _dbl, _i64, _vp, _vp]
     lib.lrmd_set_shard.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp]
     lib.lrmd_pair_sym_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
+    lib.lrmd_fp64_peak.argtypes = [_int, _int, _int, _int, _int, _vp, C.c_size_t, C.POINTER(_dbl), _vp]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int
@@ -216,6 +217,15 @@ def lrmd_pair_sym_partition(ctx):
             break
         rc = load().lrmd_pair_sym_partition(ctx, w, tab[w].ctypes.data, None)
     return rc, tab
+
+
+def lrmd_fp64_peak(op: int, mix: int, extra_per_16: int, warps_per_sm: int, iters: int, scratch_device: int,
+                   scratch_bytes: int, stream: int = 0):
+    """Diagnostic: (rc, (fp64 instr/s, SM MHz held, FP64 lanes per clock per SM, ms)) of the issue-rate microbenchmark."""
+    out = (_dbl * 4)()
+    rc = load().lrmd_fp64_peak(int(op), int(mix), int(extra_per_16), int(warps_per_sm), int(iters), scratch_device,
+                               int(scratch_bytes), out, stream)
+    return rc, tuple(float(v) for v in out)
 
 
 # ---- convenience object ---------------------------------------------------------------------------------

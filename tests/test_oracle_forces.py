@@ -245,6 +245,74 @@ def test_abs_sums_rows_and_threads(ref):
     assert np.all(S >= A * (1 - 1e-12) - 1.0 / 200)
 
 
+def _pair_potential_mp(model, eps, ai, bi, aj, bj, N):
+    """One term of the printed double sums (eq.(1), :36 eq.(2), :40 eq.(3)), with its 1/N."""
+    if model == HMF:
+        return (1 - mp.cos(ai - aj)) / N
+    if model == RING:
+        return -1 / (mp.sqrt(2) * mp.sqrt(1 - mp.cos(ai - aj) + eps)) / N
+    return mp.log((ai - aj) ** 2 + (bi - bj) ** 2 + eps) / N
+
+
+@pytest.mark.parametrize("model,eps,form", [(HMF, 0.0, 1), (RING, 0.01, 0), (RING, 0.01, 1), (RING, 1e-3, 1),
+                                            (GRAV2D, 1e-3, 0)])
+def test_abs_force_sums_every_branch(ref, model, eps, form):
+    """Pins lrmd_ref_abs_force_sums, the scale A_i = sum_{j != i} |f_ij| of every force tolerance
+    (north_star: |f_gpu - f_ref|_i <= 1e-12 A_i), for every branch that computes it: each |f_ij| is the
+    absolute value of the mpmath numerical derivative of ONE printed pair-potential term with respect to
+    particle i's coordinate — no force formula is typed here, so a dropped fabs, a wrong prefactor or a
+    swapped component in the oracle fails."""
+    N = 9
+    q0, q1 = _rand_state(model, N, 31 + model)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=form)
+    e = mp.mpf(float(eps))
+    a = [mp.mpf(float(v)) for v in q0]
+    b = [mp.mpf(0)] * N if q1 is None else [mp.mpf(float(v)) for v in q1]
+    for i in range(N):
+        ex = mp.mpf(0)
+        ey = mp.mpf(0)
+        for j in range(N):
+            if j == i:
+                continue
+            ex += abs(mp.diff(lambda z: _pair_potential_mp(model, e, z, b[i], a[j], b[j], N), a[i]))
+            if model == GRAV2D:
+                ey += abs(mp.diff(lambda z: _pair_potential_mp(model, e, a[i], z, a[j], b[j], N), b[i]))
+        assert abs(A0[i] - float(ex)) <= 1e-13 * float(ex), (i, A0[i], float(ex))
+        assert A0[i] >= abs(f0[i]) * (1 - 1e-15)
+        if model == GRAV2D:
+            assert abs(A1[i] - float(ey)) <= 1e-13 * float(ey), (i, A1[i], float(ey))
+            assert A1[i] >= abs(f1[i]) * (1 - 1e-15)
+    # sampled rows return the same A_i as the full call
+    rows = np.array([N - 1, 0, 4])
+    out = ref.forces_rows(model, eps, q0, q1, rows, form=form, with_abs=True)
+    assert np.array_equal(out[2], A0[rows])
+    if model == GRAV2D:
+        assert np.array_equal(out[3], A1[rows])
+
+
+def test_hmf_force_bound_is_pinned_from_both_sides(ref):
+    """The O(N) scale used at N = 5e7 (config 4), S_i = |cos t_i| <|sin|> + |sin t_i| <|cos|>:
+    (a) it equals that expression evaluated independently with math.fsum, to rounding — so it cannot be
+    over-generous; (b) it bounds the true A_i = (1/N) sum_{j != i} |sin(t_i - t_j)| from above (triangle
+    inequality on sin(a - b) = sin a cos b - cos a sin b), and is not far above it (<= sqrt2 A_i + 1/N for
+    angles spread over the circle)."""
+    N = 300
+    th, _ = _rand_state(HMF, N, 6)
+    _, _, S, _ = ref.forces_abs(HMF, 0.0, th, form=0)
+    mean_abs_sin = math.fsum(abs(math.sin(t)) for t in th) / N
+    mean_abs_cos = math.fsum(abs(math.cos(t)) for t in th) / N
+    for i in range(N):
+        want = abs(math.cos(th[i])) * mean_abs_sin + abs(math.sin(th[i])) * mean_abs_cos
+        assert abs(S[i] - want) <= 4e-16 * want
+        A = math.fsum(abs(math.sin(th[i] - t)) for j, t in enumerate(th) if j != i) / N
+        assert S[i] >= A * (1 - 1e-14)
+        assert S[i] <= 2.0 * A + 1.0 / N
+    # sampled rows carry the same bound
+    rows = np.array([7, 299, 0])
+    out = ref.forces_rows(HMF, 0.0, th, None, rows, form=0, with_abs=True)
+    assert np.array_equal(out[2], S[rows])
+
+
 def test_waterbag_magnetisation_statistics(ref):
     """Config-1 shaped input: theta ~ U[-1.5, 1.5) => E[M] = sin(1.5)/1.5 = 0.66500."""
     from paper_1212_0262_b200 import inputs
