@@ -83,6 +83,10 @@ enum {
                                     kernel LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, not CTAs.            */
     LRMD_OPT_PAIR_SYM_TILES = 9, /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
                                     N doubles per tile and component, within 1 GiB); get: the value in use            */
+    LRMD_OPT_PAIR_SYM_EXCHANGE = 11, /* symmetric fp64 kernel: how the j-packet (position + collected force) meets the lanes:
+                                    0 = it travels around the warp by shuffles, 1-3 = it lives in a per-warp shared-memory
+                                    buffer (register budget for 2, 3, 4 resident CTAs per SM); -1 = choose.  Results differ
+                                    between 0 and 1-3 in the rounding of the j-side sums only.                        */
     LRMD_OPT_PAIR_FUSE_UPDATE = 10 /* symmetric kernel, one launch per force evaluation: 0 = separate update kernel,
                                     1 / -1 = the kick / drift that follows a force evaluation runs inside its fold
                                     kernel (same arithmetic, bit-identical results); get: whether it is in use       */

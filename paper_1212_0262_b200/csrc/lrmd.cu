@@ -54,7 +54,7 @@ struct lrmd_ctx {
     void* coll_user = nullptr;
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
-    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0, opt_fuse = -1;
+    int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0, opt_fuse = -1, opt_sym_xch = -1;
     // resolved
     int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
     int slots = 1;              // partial force rows per particle (pair models)
@@ -65,6 +65,7 @@ struct lrmd_ctx {
     std::vector<int2> sym_tiles;
     std::vector<int4> sym_batches;   // (first tile, end tile, first worker, workers) per launch
     int sym_slots = 1, sym_R = 4, sym_rows = 1;
+    int sym_xch = 3;            // LRMD_OPT_PAIR_SYM_EXCHANGE as resolved
     bool use_graph = false;
     Layout lay;
     // bindings
@@ -190,6 +191,7 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     int smax = 1;
     for (const int2& r : c->sym_tiles) if (r.y - r.x + 1 > smax) smax = r.y - r.x + 1;
     c->sym_slots = smax;
+    c->sym_xch = c->opt_sym_xch >= 0 ? (int)c->opt_sym_xch : 3;
     c->sym_R = R;
     c->sym_rows = (int)TB;
     lrmd::SymPart S;
@@ -285,6 +287,12 @@ void resolve(lrmd_ctx* c) {
     L.kpart = off; off = align_up(off + sizeof(double) * 3 * kEnergyGrid);
     L.total = off;
     c->lay = L;
+}
+
+// After resolve(): the bound workspace stays valid only if every offset is unchanged and no device-resident work table
+// (symmetric kernel) was rebuilt; otherwise the context returns to "workspace not set" (lrmd.h, lrmd_set_workspace).
+void rebind_if_changed(lrmd_ctx* c, const Layout& before, bool had_sym) {
+    if (std::memcmp(&before, &c->lay, sizeof(Layout)) != 0 || had_sym || c->sym) c->ws = nullptr;
 }
 
 void drop_graph(lrmd_ctx* c) {
@@ -515,7 +523,8 @@ int hmf_step_cluster(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     if (t) {
         while (c->ev.size() < c->ev_used + 2) {
             cudaEvent_t e;
-            if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); return LRMD_ECUDA; }
+            const cudaError_t ee = cudaEventCreate(&e);
+            if (ee != cudaSuccess) { c->cuda_err = (int)ee; (void)cudaGetLastError(); return LRMD_ECUDA; }
             c->ev.push_back(e);
         }
         cudaEventRecord(c->ev[c->ev_used], stream);
@@ -597,12 +606,22 @@ void pair_force_sym(Launcher& L, int upd = 0, double kickA = 0.0, double kickB =
         if (c->opt_precision == 1) {
             if (c->sym_R == 8) L.go_timed(grav_force_sym_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), S, (float)c->eps, pre, i0, i1, j0, j1);
             else L.go_timed(grav_force_sym_f32_kernel<4>, g, b, (const float2*)js32_ptr(c), S, (float)c->eps, pre, i0, i1, j0, j1);
-        } else if (c->model == LRMD_RING) {
-            if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<1, 8>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
-            else L.go_timed(pair_force_sym_kernel<1, 4>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
         } else {
-            if (c->sym_R == 8) L.go_timed(pair_force_sym_kernel<2, 8>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
-            else L.go_timed(pair_force_sym_kernel<2, 4>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1);
+#define LRMD_SYM_GO(M, RR, X, MB) L.go_timed(pair_force_sym_kernel<M, RR, X, MB>, g, b, js_ptr(c), S, c->eps, pre, i0, i1, j0, j1)
+#define LRMD_SYM_X(M, RR)                                   \
+            switch (c->sym_xch) {                           \
+                case 0: LRMD_SYM_GO(M, RR, 0, 2); break;    \
+                case 1: LRMD_SYM_GO(M, RR, 1, 2); break;    \
+                case 2: LRMD_SYM_GO(M, RR, 1, 3); break;    \
+                default: LRMD_SYM_GO(M, RR, 1, 4); break;   \
+            }
+            if (c->model == LRMD_RING) {
+                if (c->sym_R == 8) { LRMD_SYM_X(1, 8) } else { LRMD_SYM_X(1, 4) }
+            } else {
+                if (c->sym_R == 8) { LRMD_SYM_X(2, 8) } else { LRMD_SYM_X(2, 4) }
+            }
+#undef LRMD_SYM_X
+#undef LRMD_SYM_GO
         }
         // rows of this batch only concern particles from its first tile on
         const long long first = (long long)S.tile0 * S.T;
@@ -716,7 +735,7 @@ int lrmd_create(lrmd_ctx** out, int model, int64_t N, double eps) {
     if (model != LRMD_HMF && N > ((int64_t)1 << 28)) return LRMD_EINVAL;   // O(N^2) models: 7e16 pairs per force
     if (model != LRMD_HMF && !finite_pos(eps)) return LRMD_EINVAL;
     lrmd_ctx* c = new (std::nothrow) lrmd_ctx();
-    if (!c) return LRMD_EINVAL;
+    if (!c) return LRMD_ESTATE;     // host allocation failed: there is no context to report on
     c->model = model;
     c->N = N;
     c->N_total = N;
@@ -910,12 +929,13 @@ int lrmd_set_shard(lrmd_ctx* c, int64_t N_total, int64_t i0, lrmd_allreduce_fn a
     c->allreduce = allreduce;
     c->allgather = allgather;
     c->coll_user = user;
-    const size_t before = c->lay.total;
+    const Layout before = c->lay;
+    const bool had_sym = c->sym;
     resolve(c);
     drop_graph(c);
     c->force_valid = false;
     c->js_valid = false;
-    if (c->lay.total > before) c->ws = nullptr;   // back to "workspace not set"
+    rebind_if_changed(c, before, had_sym);
     return LRMD_OK;
 }
 
@@ -982,6 +1002,12 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
             c->opt_sym_tiles = value;
             break;
+        case LRMD_OPT_PAIR_SYM_EXCHANGE:
+            if (value < -1 || value > 3) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
+            c->opt_sym_xch = value;
+            c->sym_xch = value >= 0 ? (int)value : 3;
+            return LRMD_OK;
         case LRMD_OPT_KERNEL_TIMING:
             if (value != 0 && value != 1) return LRMD_EINVAL;
             c->timing = value != 0;
@@ -990,12 +1016,13 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
         default:
             return LRMD_EINVAL;
     }
-    const size_t before = c->lay.total;
+    const Layout before = c->lay;
+    const bool had_sym = c->sym;
     resolve(c);
     drop_graph(c);
     c->force_valid = false;
     c->js_valid = false;
-    if (c->lay.total > before) c->ws = nullptr;   // back to "workspace not set"
+    rebind_if_changed(c, before, had_sym);
     return LRMD_OK;
 }
 
@@ -1013,6 +1040,7 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;
+        case LRMD_OPT_PAIR_SYM_EXCHANGE: *value = c->sym ? c->sym_xch : 0; break;
         default: return LRMD_EINVAL;
     }
     return LRMD_OK;

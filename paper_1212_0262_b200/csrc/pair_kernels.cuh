@@ -469,12 +469,108 @@ __device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b
     }
 }
 
+// The same walk with the packet held in shared memory instead of travelling by shuffles (one 1 KB buffer per
+// warp): lane l owns slot l (position of j = 32 c + l and the force that j collects); in step s every lane works
+// on slot (l + s) mod 32 — one conflict-free LDS.128 for the position, and the slot's force sum is read, extended
+// by the lane's R pair terms and written back (LDS.128 / STS.128); __syncwarp() orders a step's write-back before
+// the neighbour lane's read of the same slot in the next step.  Measured on B200 with lrmd_fp64_peak
+// (profiles/r02_fp64_peak.md): next to DFMA traffic an LDS / STS / integer instruction costs no FP64 issue
+// cycle, a SHFL costs about one (the shuffle walk spends 8 per step), and the position of the next step no longer
+// depends on a shuffle chain.
+struct SymWarpSmem {
+    double2 pos[32];
+    double2 g[32];
+};
+
+template <int MODEL, int R, bool MASK, bool DIAG>
+__device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const double (&b)[R], const bool (&vi)[R],
+                                               double (&f0)[R], double (&f1)[R], SymWarpSmem& sw, int nvalid, double eps,
+                                               double onepe) {
+    const int lane = threadIdx.x & 31;
+    double2 qn = sw.pos[lane];
+#pragma unroll 8
+    for (int s = 0; s < 32; ++s) {
+        const int idx = (lane + s) & 31;
+        const double2 q = qn;
+        qn = sw.pos[(idx + 1) & 31];                 // next step's position, loaded a step ahead
+        double h0 = 0.0, h1 = 0.0;
+        if (!DIAG) {                                 // the slot's force sum so far
+            const double2 g = sw.g[idx];
+            h0 = g.x;
+            h1 = g.y;
+        }
+        const bool vq = MASK ? (idx < nvalid) : true;
+#pragma unroll
+        for (int r0 = 0; r0 < R; r0 += 4) {
+            if (MODEL == 2) {
+                double dx[4], dy[4], r2[4], y0[4], y[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    dx[k] = a[r0 + k] - q.x;
+                    dy[k] = b[r0 + k] - q.y;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) r2[k] = fma(dy[k], dy[k], fma(dx[k], dx[k], eps));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y0[k] = rcp_seed(r2[k]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double e = fma(-r2[k], y0[k], 1.0);
+                    y[k] = fma(e, e, e);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    y[k] = fma(y0[k], y[k], y0[k]);
+                    if (MASK) y[k] = (vi[r0 + k] && vq) ? y[k] : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    f0[r0 + k] = fma(dx[k], y[k], f0[r0 + k]);
+                    if (!DIAG) h0 = fma(-dx[k], y[k], h0);
+                    f1[r0 + k] = fma(dy[k], y[k], f1[r0 + k]);
+                    if (!DIAG) h1 = fma(-dy[k], y[k], h1);
+                }
+            } else {
+                double num[4], d[4], y0[4], c[4], p[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    num[k] = fma(b[r0 + k], q.x, -(a[r0 + k] * q.y));                 // s_i c_j - c_i s_j
+                    d[k] = fma(-b[r0 + k], q.y, fma(-a[r0 + k], q.x, onepe));      // 1 + eps - c_i c_j - s_i s_j
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) y0[k] = rsqrt_seed(d[k]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double bb = y0[k] * y0[k];
+                    const double e = fma(-d[k], bb, 1.0);
+                    c[k] = (num[k] * y0[k]) * bb;
+                    p[k] = fma(fma(1.875, e, 1.5), e, 1.0);
+                    if (MASK) c[k] = (vi[r0 + k] && vq) ? c[k] : 0.0;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    f0[r0 + k] = fma(c[k], p[k], f0[r0 + k]);
+                    if (!DIAG) h0 = fma(-c[k], p[k], h0);
+                }
+            }
+        }
+        if (!DIAG) {
+            sw.g[idx] = make_double2(h0, h1);
+            __syncwarp();
+        }
+    }
+}
+
 // (launch bound of 2 CTAs per SM: with the full register budget ptxas interleaves the pair chains of a step —
 //  184-255 registers instead of 140 — which is worth 5-6 % although only 8 warps per SM stay resident)
-template <int MODEL, int R>
-__global__ void __launch_bounds__(kSymThreads, 2)
+// XCH: 0 = the packet travels by shuffles, 1 = it lives in shared memory (sym_chunk_smem); MINB = resident CTAs per SM
+// the register budget is set for.
+template <int MODEL, int R, int XCH, int MINB>
+__global__ void __launch_bounds__(kSymThreads, MINB)
 pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, double pre, double* __restrict__ ipart0,
                       double* __restrict__ ipart1, double* __restrict__ jpart0, double* __restrict__ jpart1) {
+    __shared__ SymWarpSmem swarp[XCH ? kSymThreads / 32 : 1];
+    SymWarpSmem& sw = swarp[XCH ? (threadIdx.x >> 5) : 0];
     const int w = blockIdx.x * (kSymThreads / 32) + (threadIdx.x >> 5);
     if (w >= S.G) return;
     const int lane = threadIdx.x & 31;
@@ -488,6 +584,7 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
     bool vi[R];
     unsigned selfmask = 0u;   // rows whose own chunk this worker walked since load_tile (Ring: self term to remove)
     auto load_tile = [&](int t) {
+        selfmask = 0u;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const long long i = (long long)t * S.T + r * 32 + lane;
@@ -536,13 +633,36 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
         double g0 = 0.0, g1 = 0.0;
         const bool diag = cchunk < (ctile + 1) * R;
         const bool masked = ragged && (ctile == S.ntiles - 1 || cchunk == S.nchunks - 1);
+        if (XCH) {
+            const long long left = N - (long long)cchunk * 32;
+            const int nvalid = left < 32 ? (int)left : 32;
+            sw.pos[lane] = q;
+            sw.g[lane] = make_double2(0.0, 0.0);
+            __syncwarp();
+            if (diag) {
+                if (masked) sym_chunk_smem<MODEL, R, true, true>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+                else sym_chunk_smem<MODEL, R, false, true>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+            } else {
+                if (masked) sym_chunk_smem<MODEL, R, true, false>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+                else sym_chunk_smem<MODEL, R, false, false>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+            }
+            __syncwarp();
+            const double2 g = sw.g[lane];
+            g0 = g.x;
+            g1 = g.y;
+            __syncwarp();      // every lane has read its slot before the next unit overwrites the buffer
+        }
         if (diag) {
-            if (masked) sym_chunk<MODEL, R, true, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
-            else sym_chunk<MODEL, R, false, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            if (!XCH) {
+                if (masked) sym_chunk<MODEL, R, true, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+                else sym_chunk<MODEL, R, false, true>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            }
             selfmask |= 1u << (cchunk - ctile * R);   // this walk met j = i for that row of every lane (step 0)
         } else {
-            if (masked) sym_chunk<MODEL, R, true, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
-            else sym_chunk<MODEL, R, false, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            if (!XCH) {
+                if (masked) sym_chunk<MODEL, R, true, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+                else sym_chunk<MODEL, R, false, false>(a, b, vi, f0, f1, q, vq, eps, onepe, g0, g1);
+            }
             if (vq) {
                 jpart0[(long long)(ctile - S.tile0) * N + j] = pre * g0;
                 if (MODEL == 2) jpart1[(long long)(ctile - S.tile0) * N + j] = pre * g1;

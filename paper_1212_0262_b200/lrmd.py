@@ -20,6 +20,7 @@ OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED, ECOLL = 0, -1, -2, -3, -4, -5
 OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
 OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS, OPT_PAIR_SYMMETRIC, OPT_PAIR_SYM_TILES = 5, 6, 7, 8, 9
 OPT_PAIR_FUSE_UPDATE = 10
+OPT_PAIR_SYM_EXCHANGE = 11
 
 #: every symbol include/lrmd.h declares (tests check the library exports each of them)
 SYMBOLS = (
@@ -280,7 +281,7 @@ class Context:
 
     def set_option(self, key: int, value: int):
         self._chk(lrmd_set_option(self._h, key, value), "lrmd_set_option")
-        if key not in (OPT_KERNEL_TIMING, OPT_PAIR_FUSE_UPDATE):   # the others may change the workspace size
+        if key not in (OPT_KERNEL_TIMING, OPT_PAIR_FUSE_UPDATE, OPT_PAIR_SYM_EXCHANGE):   # the others may change the workspace size
             self._bind_workspace()
 
     def get_option(self, key: int) -> int:

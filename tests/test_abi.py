@@ -266,3 +266,49 @@ def test_kernel_sincos_special_points_mpmath(lrmd):
     assert s[0] == 0.0 and c[0] == 1.0
     sn, cn = lrmd.lrmd_host_sincos(np.array([float("nan"), float("inf")]))
     assert np.all(np.isnan(sn)) and np.all(np.isnan(cn))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("how", ["set_option", "set_shard"])
+def test_reresolving_a_symmetric_context_unbinds_the_workspace(lrmd, how):
+    """Raw C ABI, no Context object: a RING context with N = 4096 uses the symmetric kernel, whose work tables live in
+    the workspace.  lrmd_set_option / lrmd_set_shard after lrmd_set_workspace rebuild those tables on the host, so the
+    context must return to 'workspace not set' (LRMD_ESTATE) instead of launching with stale table pointers; after a
+    re-bind the step runs and matches a fresh context bit for bit."""
+    import numpy as np
+    import torch
+    assert torch.cuda.is_available()
+    N = 4096
+    rng = np.random.default_rng(5)
+    th0, p0 = rng.uniform(-1, 1, N), rng.uniform(-0.3, 0.3, N)
+
+    def fresh():
+        rc, h = lrmd.lrmd_create(RING, N, 0.01)
+        assert rc == lrmd.OK
+        rc, nbytes = lrmd.lrmd_workspace_bytes(h)
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        ptr = (ws.data_ptr() + 255) // 256 * 256
+        assert lrmd.lrmd_set_workspace(h, ptr, nbytes) == lrmd.OK
+        th = torch.tensor(th0, device="cuda")
+        p = torch.tensor(p0, device="cuda")
+        assert lrmd.lrmd_set_state(h, th.data_ptr(), p.data_ptr()) == lrmd.OK
+        return h, ws, ptr, nbytes, th, p
+
+    h, ws, ptr, nbytes, th, p = fresh()
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SYMMETRIC) == (lrmd.OK, 1)
+    if how == "set_option":
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_GRAPH, 0) == lrmd.OK
+    else:
+        assert lrmd.load().lrmd_set_shard(h, N, 0, None, None, None) == lrmd.OK
+    assert lrmd.lrmd_step(h, 1, 0.01) == lrmd.ESTATE
+    rc, nbytes2 = lrmd.lrmd_workspace_bytes(h)
+    assert rc == lrmd.OK and nbytes2 <= nbytes
+    assert lrmd.lrmd_set_workspace(h, ptr, nbytes) == lrmd.OK
+    assert lrmd.lrmd_step(h, 2, 0.01) == lrmd.OK
+    torch.cuda.synchronize()
+    h2, ws2, _, _, th2, p2 = fresh()
+    assert lrmd.lrmd_step(h2, 2, 0.01) == lrmd.OK
+    torch.cuda.synchronize()
+    assert torch.equal(th, th2) and torch.equal(p, p2)
+    lrmd.lrmd_destroy(h)
+    lrmd.lrmd_destroy(h2)
