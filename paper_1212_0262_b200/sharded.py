@@ -72,9 +72,22 @@ class ShardedContext(lrmd.Context):
             raise RuntimeError("collective buffer outside the workspace")
         return self._ws[off:off + nbytes]
 
+    def _on_stream(self, stream):
+        """Context manager that makes ``stream`` (the raw cudaStream_t the library launches its kernels on) torch's
+        current stream, so that a ``torch.distributed`` collective issued inside is ordered after the kernels
+        already enqueued on it and before the ones that follow (the process group orders its work against the
+        current stream).  CPU tensors (gloo tests) have no stream: a null context."""
+        import contextlib
+        torch = self._torch
+        if self._ws.device.type != "cuda":
+            return contextlib.nullcontext()
+        ext = torch.cuda.ExternalStream(int(stream or 0), device=self._ws.device)
+        return torch.cuda.stream(ext)
+
     def _allreduce(self, ptr, count, stream, user):
         try:
-            self.coll.all_reduce_sum_(self._view(ptr, 8 * count).view(self._torch.float64))
+            with self._on_stream(stream):
+                self.coll.all_reduce_sum_(self._view(ptr, 8 * count).view(self._torch.float64))
             return 0
         except Exception:          # never let an exception cross the C boundary
             return 1
@@ -82,7 +95,8 @@ class ShardedContext(lrmd.Context):
     def _allgather(self, ptr, elem_bytes, i0, n_local, n_total, stream, user):
         try:
             whole = self._view(ptr, elem_bytes * n_total)
-            self.coll.all_gather_inplace_(whole, [(b * elem_bytes, (b + n) * elem_bytes) for b, n in self.bounds])
+            with self._on_stream(stream):
+                self.coll.all_gather_inplace_(whole, [(b * elem_bytes, (b + n) * elem_bytes) for b, n in self.bounds])
             return 0
         except Exception:
             return 1
