@@ -76,17 +76,22 @@ enum {
     LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
                                     of the pair kernels (-1 = choose)                                          */
     LRMD_OPT_PAIR_SLOTS = 7,     /* read-only (lrmd_get_option): partial force rows per particle          */
-    LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models, fp64: 1 = force kernel that evaluates every UNORDERED pair once and adds
-                                    +f / -f to both particles (the paper declines this);
-                                    0 = every ordered pair (the paper's scheme); -1 = choose (symmetric for N >= 2048
-                                    unless the context is a shard).  With the symmetric
-                                    kernel LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, not CTAs.            */
+    LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models: force kernels that evaluate every UNORDERED pair once and add +f / -f to
+                                    both particles (the paper declines this): 1 = warp-level
+                                    kernel (one j-side scratch row per 32R-particle tile; fp64 and, GRAV2D, fp32 pairs),
+                                    2 = band kernel (fp64 only; both sides' sums kept on chip over blocks of 8 x 32R
+                                    particles, one launch for any N, about 25 N doubles of scratch per component);
+                                    0 = every ordered pair (the paper's scheme); -1 = choose (1 for 2048 <= N < 49,152,
+                                    2 beyond, 0 if the context is a shard).  get: the kernel in use.  With 1
+                                    LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, with 2 CTAs.                */
     LRMD_OPT_PAIR_SYM_TILES = 9, /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
                                     N doubles per tile and component, within 1 GiB); get: the value in use            */
     LRMD_OPT_PAIR_SYM_EXCHANGE = 11, /* symmetric fp64 kernel: how the j-packet (position + collected force) meets the lanes:
                                     0 = it travels around the warp by shuffles, 1-3 = it lives in a per-warp shared-memory
                                     buffer (register budget for 2, 3, 4 resident CTAs per SM); -1 = choose.  Results differ
                                     between 0 and 1-3 in the rounding of the j-side sums only.                        */
+    LRMD_OPT_PAIR_BAND_HEIGHT = 12, /* band kernel: I-blocks per band (0 = choose: the height that minimises the scratch
+                                    rows); get: the value in use                                                      */
     LRMD_OPT_PAIR_FUSE_UPDATE = 10 /* symmetric kernel, one launch per force evaluation: 0 = separate update kernel,
                                     1 / -1 = the kick / drift that follows a force evaluation runs inside its fold
                                     kernel (same arithmetic, bit-identical results); get: whether it is in use       */
@@ -213,6 +218,13 @@ int lrmd_fp64_peak(int op, int mix, int extra_per_16, int warps_per_sm, int iter
  * `cta` as rows {tile, jbeg, jend, slot} (4 int64 each, at most max_seg rows) and their number to
  * *nseg_host: the CTA adds the pairs (i in tile) x (jbeg <= j < jend) into partial force row `slot`. */
 int lrmd_pair_partition(const lrmd_ctx* ctx, int64_t cta, int64_t* seg4_host, int64_t max_seg, int64_t* nseg_host);
+
+/* Diagnostic (HOST pointers, no GPU needed): the work partition of the band kernel (LRMD_OPT_PAIR_SYMMETRIC = 2).
+ * Particles are grouped into I-blocks of IB rows and these into bands; band A's work is every pair (i in the band,
+ * j >= the band's first row), cut into column ranges ("pieces").  *n_pieces_host (if not NULL) receives the number of
+ * pieces (0 if the band kernel is not in use); out8_host (if not NULL) receives, for piece `piece`,
+ * {band, c0, c1 (columns [32 c0, 32 c1)), owning worker, first I-block of the band, I-blocks in the band, IB, workers}. */
+int lrmd_pair_band_partition(const lrmd_ctx* ctx, int64_t piece, int64_t* out8_host, int64_t* n_pieces_host);
 
 /* Diagnostic (HOST pointers, no GPU needed): the work table of the symmetric pair kernel (LRMD_OPT_PAIR_SYMMETRIC).
  * Work units are (i-tile, chunk of 32 j) pairs with chunk >= tile * (tile size / 32), in tile-major order; each

@@ -1,0 +1,226 @@
+// band_kernels.cuh — Newton's-third-law force kernel for large N (PAPER.md:108 is the passage it
+// overturns): the warp-systolic walk of pair_kernels.cuh (sym_chunk_smem) inside a two-level blocking that keeps BOTH
+// sides' partial sums on chip, so that one launch serves any N and the scratch rows shrink from N^2 / 256 doubles per
+// component (one j-side row per 256-particle tile) to about 25 N.
+//
+//   * A CTA of 8 warps holds an I-block of IB = 8 x 32 R particles in registers (R per lane, as before) and a J-block
+//     of IB particles in shared memory: positions (TMA bulk copy) and the force sums they collect.  The 8 warps walk
+//     the J-block's 32-particle chunks at staggered offsets; a chunk's force sums stay in shared memory from one warp's
+//     visit to the next, so the j-side sum of the whole I-block is formed on chip.  CTA barriers every n / 8 chunk
+//     walks keep the visits to a chunk in a fixed order: deterministic, no atomics.
+//   * I-blocks are grouped into bands of hb consecutive blocks.  The work of band A — all columns from the band's first
+//     row to N — is cut into contiguous column ranges ("pieces") of equal weight, one or two per CTA.  For every
+//     J-block of its piece a CTA loops over the band's I-blocks: the J-block's sums meet hb x IB rows before they are
+//     written to the band's j-side row jbuf[band][column] (written once per band and column); the i-side sums of an
+//     I-block are added to the piece's private row ibuf[piece][row] (one read-modify-write per J-block, private to the
+//     CTA, in J-block order).
+//   * The J-block that holds the I-block's own rows is walked in DIAG mode by every warp (i-side only, each ordered
+//     pair of the block once): all warps carry the same load; J-blocks below it are skipped (their pairs are met from
+//     the other side).
+//   * pair_band_fold_kernel adds, for particle i, the i-side rows of its band's pieces and the j-side rows of the bands
+//     up to its own, in a fixed order, and applies the kick / drift that follows (as pair_sym_fold_kernel does).
+#pragma once
+
+#include "pair_kernels.cuh"
+
+namespace lrmd {
+
+constexpr int kBandWarps = 8;
+constexpr int kBandThreads = 32 * kBandWarps;
+
+struct BandPiece {
+    int band;       // band the piece belongs to
+    int c0, c1;     // its columns, in chunks of 32 particles: [c0, c1)
+    int pad;
+};
+struct BandInfo {
+    int blk0, nblk;     // I-blocks blk0 .. blk0 + nblk - 1
+    int pf0, pf1;       // pieces pf0 .. pf1 - 1, in column order
+    long long joff;     // offset (elements) of the band's j-side row: column col is at joff + col - 32 cstart
+    int cstart;         // first column chunk of the band = blk0 * IB / 32
+    int pad;
+};
+struct BandPart {
+    long long N;
+    long long istride;  // rows of a full band = hb * IB: stride between the pieces' i-side rows
+    int IB;             // rows per I-block = columns per J-block = kBandWarps * 32 * R
+    int nIB, nchunks, nbands, hb;
+    int P;              // workers (CTAs)
+    const int* wpiece;          // [P + 1] first piece of every worker
+    const BandPiece* pieces;
+    const BandInfo* bands;
+};
+
+// dynamic shared memory: positions and force sums of one J-block + one mbarrier
+constexpr size_t band_smem_bytes(int R) { return (size_t)2 * kBandWarps * 32 * R * sizeof(double2) + 16; }
+
+template <int MODEL, int R>
+__global__ void __launch_bounds__(kBandThreads, 2)
+pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, double pre, double* __restrict__ ibuf0,
+                       double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1) {
+    extern __shared__ __align__(128) unsigned char band_smem[];
+    constexpr int T = 32 * R;                 // rows per warp tile
+    constexpr int IB = kBandWarps * T;        // rows per I-block, columns per J-block
+    constexpr int JB = IB / 32;               // chunks per J-block
+    double2* Jpos = reinterpret_cast<double2*>(band_smem);
+    double2* Jg = Jpos + IB;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(Jg + IB);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long N = B.N;
+    const double onepe = 1.0 + eps;
+    const bool ragged = (N % T) != 0;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0u;
+
+    const int pfirst = B.wpiece[blockIdx.x], plast = B.wpiece[blockIdx.x + 1];
+    for (int pc = pfirst; pc < plast; ++pc) {
+        const BandPiece piece = B.pieces[pc];
+        const BandInfo band = B.bands[piece.band];
+        const int jbfirst = piece.c0 / JB;
+        for (int jb = jbfirst; jb * JB < piece.c1; ++jb) {
+            const int jc0 = piece.c0 > jb * JB ? piece.c0 : jb * JB;
+            const int jc1 = piece.c1 < (jb + 1) * JB ? piece.c1 : (jb + 1) * JB;
+            const int n = jc1 - jc0;                               // chunks of this J-block segment
+            const long long col0 = (long long)jc0 * 32;
+            const int ncol = (int)((N - col0 < (long long)n * 32) ? (N - col0) : (long long)n * 32);   // columns that exist
+            __syncthreads();    // the previous segment's shared-memory reads are done
+            if (threadIdx.x == 0) {
+                mbar_expect_tx(bar, (uint32_t)ncol * (uint32_t)sizeof(double2));
+                bulk_g2s(Jpos, js + col0, (uint32_t)ncol * (uint32_t)sizeof(double2), bar);
+            }
+            for (int x = threadIdx.x; x < n * 32; x += kBandThreads) {
+                Jg[x] = make_double2(0.0, 0.0);
+                if (x >= ncol) Jpos[x] = make_double2(0.0, 0.0);
+            }
+            mbar_wait(bar, phase);
+            phase ^= 1u;
+            __syncthreads();
+
+            // virtual chunk count: with fewer than 8 chunks the warps take turns (one warp per chunk at a time)
+            const int nv = n >= kBandWarps ? n : kBandWarps;
+            const int off = (warp * nv) / kBandWarps;
+            const int m = nv / kBandWarps;                          // barrier period: visits to a chunk are >= m walks apart
+            const int blk_end = band.blk0 + band.nblk < jb + 1 ? band.blk0 + band.nblk : jb + 1;
+            for (int b = band.blk0; b < blk_end; ++b) {
+                const bool diag = b == jb;
+                const int tile = b * kBandWarps + warp;
+                const bool tile_any = (long long)tile * T < N;
+                const bool masked_tile = ragged && (long long)(tile + 1) * T > N;
+                double a[R], bb[R], f0[R], f1[R];
+                bool vi[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const long long i = (long long)tile * T + r * 32 + lane;
+                    vi[r] = i < N;
+                    const double2 q = vi[r] ? js[i] : make_double2(0.0, 0.0);
+                    a[r] = q.x;
+                    bb[r] = q.y;
+                    f0[r] = 0.0;
+                    f1[r] = 0.0;
+                }
+                unsigned selfmask = 0u;
+                for (int k = 0; k < nv; ++k) {
+                    int x = k + off;
+                    if (x >= nv) x -= nv;
+                    if (tile_any && x < n) {
+                        const int gc = jc0 + x;                       // global chunk index
+                        const long long left = N - (long long)gc * 32;
+                        const int nvalid = left < 32 ? (int)left : 32;
+                        const bool masked = masked_tile || nvalid < 32;
+                        const double2* sp = Jpos + x * 32;
+                        double2* sg = Jg + x * 32;
+                        if (diag) {
+                            if (masked) sym_chunk_smem<MODEL, R, true, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                            else sym_chunk_smem<MODEL, R, false, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                            const int rr = gc - tile * R;             // the walk met j = i for row rr of every lane
+                            if (MODEL == 1 && rr >= 0 && rr < R) selfmask |= 1u << rr;
+                        } else {
+                            if (masked) sym_chunk_smem<MODEL, R, true, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                            else sym_chunk_smem<MODEL, R, false, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                        }
+                    }
+                    if (!diag && (k + 1) % m == 0 && k + 1 < nv) __syncthreads();
+                }
+                // i-side sums of this (J-block, I-block) visit -> the piece's private row (first visit stores)
+                const bool first = jb == (b > jbfirst ? b : jbfirst);
+                const long long rbase = (long long)pc * B.istride - (long long)band.blk0 * IB;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const long long i = (long long)tile * T + r * 32 + lane;
+                    if (MODEL == 1 && ((selfmask >> r) & 1u)) {
+                        // remove the rounding-level j = i term of eq.(9) again (the rounded product: N = 1 gives exactly 0)
+                        double c, p;
+                        ring_pair_parts(a[r], bb[r], make_double2(a[r], bb[r]), onepe, c, p);
+                        f0[r] -= __dmul_rn(c, p);
+                    }
+                    if (vi[r]) {
+                        double v0 = pre * f0[r];
+                        if (!first) v0 += ibuf0[rbase + i];
+                        ibuf0[rbase + i] = v0;
+                        if (MODEL == 2) {
+                            double v1 = pre * f1[r];
+                            if (!first) v1 += ibuf1[rbase + i];
+                            ibuf1[rbase + i] = v1;
+                        }
+                    }
+                }
+                __syncthreads();    // this I-block's walks are done before the next one's (fixed order of the j-side sums)
+            }
+            // the J-block segment's force sums -> the band's j-side row
+            const long long jbase = band.joff + col0 - (long long)band.cstart * 32;
+            for (int x = threadIdx.x; x < ncol; x += kBandThreads) {
+                const double2 g = Jg[x];
+                jbuf0[jbase + x] = pre * g.x;
+                if (MODEL == 2) jbuf1[jbase + x] = pre * g.y;
+            }
+        }
+    }
+}
+
+// out0 / out1[i] = the force on particle i from one launch of pair_force_band_kernel; then the update (UPD as in
+// pair_sym_fold_kernel).  Block = 32 particles x kFoldGroups term groups; terms of particle i, in this order:
+// the i-side rows of its band's pieces that reached its I-block, then the j-side rows of bands 0 .. its own.
+template <int MODEL, int UPD>
+__global__ void __launch_bounds__(32 * kFoldGroups)
+pair_band_fold_kernel(BandPart B, const double* __restrict__ ibuf0, const double* __restrict__ ibuf1,
+                      const double* __restrict__ jbuf0, const double* __restrict__ jbuf1, double* __restrict__ out0,
+                      double* __restrict__ out1, FusedUpdate U) {
+    constexpr int GR = kFoldGroups;
+    __shared__ double sf[GR][32], sg[GR][32];
+    const long long N = B.N;
+    const long long i = (long long)blockIdx.x * 32 + threadIdx.x;
+    const int k = threadIdx.y;
+    double f = 0.0, g = 0.0;
+    if (i < N) {
+        const int b = (int)(i / B.IB);
+        const int A = b / B.hb;
+        const BandInfo band = B.bands[A];
+        const int ni = band.pf1 - band.pf0;
+        const int nt = ni + A + 1;
+        for (int t = k; t < nt; t += GR) {
+            if (t < ni) {
+                const int pc = band.pf0 + t;
+                if ((long long)B.pieces[pc].c1 * 32 > (long long)b * B.IB) {       // the piece has columns at or beyond block b
+                    const long long idx = (long long)pc * B.istride + i - (long long)band.blk0 * B.IB;
+                    f += ibuf0[idx];
+                    if (MODEL == 2) g += ibuf1[idx];
+                }
+            } else {
+                const BandInfo bj = B.bands[t - ni];
+                const long long idx = bj.joff + i - (long long)bj.cstart * 32;
+                f += jbuf0[idx];
+                if (MODEL == 2) g += jbuf1[idx];
+            }
+        }
+    }
+    sf[k][threadIdx.x] = f;
+    sg[k][threadIdx.x] = g;
+    __syncthreads();
+    if (k == 0 && i < N) fold_finish<MODEL, UPD>(sf, sg, i, true, out0, out1, U);
+}
+
+}  // namespace lrmd

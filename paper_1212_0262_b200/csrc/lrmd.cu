@@ -14,6 +14,7 @@
 
 #include "hmf_kernels.cuh"
 #include "pair_kernels.cuh"
+#include "band_kernels.cuh"
 #include "peak_kernels.cuh"
 
 namespace {
@@ -38,6 +39,7 @@ struct Layout {
     size_t vpart = 0;         // one per CTA of the pair-energy kernel
     size_t shared2 = 0;       // HMF shard: this rank's (sum cos, sum sin), all-reduced in place
     size_t sym_wstart = 0, sym_tiles = 0, ipart0 = 0, ipart1 = 0, jpart0 = 0, jpart1 = 0;   // symmetric kernel
+    size_t band_wpiece = 0, band_pieces = 0, band_infos = 0, bibuf0 = 0, bibuf1 = 0, bjbuf0 = 0, bjbuf1 = 0;   // band kernel
     size_t total = 0;
 };
 
@@ -55,6 +57,7 @@ struct lrmd_ctx {
     // options as set (0 / -1 = choose)
     int64_t opt_precision = 0, opt_pair_ctas = 0, opt_graph = -1, opt_hmf_grid = 0;
     int64_t opt_hmf_variant = -1, opt_pair_variant = -1, opt_sym = -1, opt_sym_tiles = 0, opt_fuse = -1, opt_sym_xch = -1;
+    int64_t opt_band_height = 0;
     // resolved
     int hmf_grid = 0, hmf_variant = 0, pair_variant = 0;
     int slots = 1;              // partial force rows per particle (pair models)
@@ -66,6 +69,14 @@ struct lrmd_ctx {
     std::vector<int4> sym_batches;   // (first tile, end tile, first worker, workers) per launch
     int sym_slots = 1, sym_R = 4, sym_rows = 1;
     int sym_xch = 3;            // LRMD_OPT_PAIR_SYM_EXCHANGE as resolved
+    bool band = false;          // band kernel (band_kernels.cuh) in use for the force; the tables below are uploaded
+    lrmd::BandPart bpart{};     //   by lrmd_set_workspace
+    std::vector<int> band_wpiece;
+    std::vector<lrmd::BandPiece> band_pieces;
+    std::vector<lrmd::BandInfo> band_infos;
+    std::vector<int> band_owner;     // worker of every piece (diagnostics)
+    int band_R = 8;
+    size_t band_jrow = 0;       // elements of all bands' j-side rows
     bool use_graph = false;
     Layout lay;
     // bindings
@@ -122,7 +133,9 @@ void with_pair_cfg(int v, F f) {
 
 // Symmetric force kernel (row N4): decide whether it is used and build its work tables.
 // Units are (tile, chunk) pairs in tile-major order, chunk >= tile * R; G workers get equal contiguous shares.
-void resolve_sym(lrmd_ctx* c, int /*minb*/) {
+void resolve_sym(lrmd_ctx* c, bool rows_needed) {
+    // rows_needed = false: the band kernel evaluates the force; the tables built here then serve the symmetric
+    // potential-energy kernel only (one launch, no partial force rows)
     c->sym = false;
     c->sym_wstart.clear();
     c->sym_tiles.clear();
@@ -140,13 +153,15 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     // N ~ 1.8e5 (2D), 64 batches at N = 2^20.
     int64_t TB = (int64_t)(kSymRowBytes / ((double)N * 8.0 * comps));
     if (c->opt_sym_tiles > 0) TB = c->opt_sym_tiles;
+    if (!rows_needed) TB = ntiles;
     if (TB < 1) TB = 1;
     if (TB > ntiles) TB = ntiles;
     // workers per launch: 32 per SM (4 waves of the 8 resident warps; sweeps in profiles/); at least two units each
     int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * 32;
     // the host-built work table has one entry per worker and launch: keep it below 2^22 entries (64 MB)
     const int64_t nbatches = (ntiles + TB - 1) / TB;
-    if (c->opt_pair_ctas <= 0) {
+    if (!rows_needed) Gwant = (int64_t)kNumSm * 32;
+    if (c->opt_pair_ctas <= 0 && rows_needed) {
         // a tile's i-side rows number about workers / tiles per launch: keep them within ~4 GiB
         int64_t maxslots = (int64_t)(4.0 * 1073741824.0 / ((double)N * 8.0 * comps));
         if (maxslots < 8) maxslots = 8;
@@ -165,7 +180,7 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
         int64_t U = 0;
         for (int64_t a = t0; a < t1; ++a) U += nchunks - a * R;
         int64_t G = Gwant;
-        if (c->opt_pair_ctas <= 0 && G > U / 2) G = U / 2;
+        if ((c->opt_pair_ctas <= 0 || !rows_needed) && G > U / 2) G = U / 2;
         if (G > U) G = U;
         if (G < 1) G = 1;
         const int64_t w0 = (int64_t)c->sym_wstart.size();
@@ -199,6 +214,109 @@ void resolve_sym(lrmd_ctx* c, int /*minb*/) {
     S.wstart = nullptr; S.tile_rng = nullptr;
     c->spart = S;
     c->sym = true;
+}
+
+// Band kernel (band_kernels.cuh): choose the band height, cut every band's columns into pieces of equal weight and
+// assign them to the P workers in band-major order.  Weight of one 32-column chunk in column block blk of band A:
+// 11 (2D) or 12 (Ring) FP64 instructions per pair for every I-block of the band above the block, 9 / 11 for the block
+// itself if it is in the band (DIAG walk: every ordered pair, i-side only).
+constexpr int64_t kBandMinN = 49152;     // default: band kernel from this N on (unsharded fp64 contexts)
+
+void resolve_band(lrmd_ctx* c) {
+    c->band = false;
+    c->band_wpiece.clear();
+    c->band_pieces.clear();
+    c->band_infos.clear();
+    c->band_owner.clear();
+    const int64_t N = c->N;
+    if (c->opt_sym == 0 || c->opt_sym == 1 || c->N_total != c->N || c->opt_precision != 0) return;
+    if (c->opt_sym < 0 && N < kBandMinN) return;
+    const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
+    const int64_t IB = (int64_t)kBandWarps * 32 * R, JB = IB / 32;
+    const int64_t nIB = (N + IB - 1) / IB, nchunks = (N + 31) / 32;
+    if (nIB > (1 << 20)) return;
+    const int64_t P = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : 2 * (int64_t)kNumSm;
+    // band height: the i-side rows cost (pieces ~ P + bands) x hb x IB elements, the j-side rows ~ bands x N / 2
+    int64_t hb = 1;
+    if (c->opt_band_height > 0) {
+        hb = c->opt_band_height < nIB ? c->opt_band_height : nIB;
+    } else {
+        double best = -1.0;
+        for (int64_t h = 1; h <= nIB; ++h) {
+            const double nb = (double)((nIB + h - 1) / h);
+            const double cost = ((double)P + nb) * (double)h * (double)IB + nb * 0.5 * (double)N;
+            if (best < 0.0 || cost < best) { best = cost; hb = h; }
+        }
+    }
+    const int64_t nbands = (nIB + hb - 1) / hb;
+    const int64_t wsym = c->model == LRMD_RING ? 12 : 11, wdiag = c->model == LRMD_RING ? 11 : 9;
+    auto chunk_weight = [&](int64_t blk0, int64_t nblk, int64_t blk) {
+        int64_t nsym = blk - blk0 < nblk ? blk - blk0 : nblk;
+        return wsym * nsym + (blk < blk0 + nblk ? wdiag : 0);
+    };
+    double wtot = 0.0;      // exact in double: below 2^53 for every N the pair models accept
+    for (int64_t A = 0; A < nbands; ++A) {
+        const int64_t blk0 = A * hb, nblk = blk0 + hb <= nIB ? hb : nIB - blk0;
+        for (int64_t blk = blk0; blk < nIB; ++blk) {
+            const int64_t cb = blk * JB, ce = (blk + 1) * JB < nchunks ? (blk + 1) * JB : nchunks;
+            wtot += (double)(chunk_weight(blk0, nblk, blk) * (ce - cb));
+        }
+    }
+    c->band_wpiece.assign((size_t)P + 1, 0);
+    int64_t w = 0;
+    double cum = 0.0;
+    auto boundary = [&](int64_t k) { return std::floor(wtot * (double)k / (double)P); };
+    double next = boundary(1);
+    size_t jrow = 0;
+    for (int64_t A = 0; A < nbands; ++A) {
+        const int64_t blk0 = A * hb, nblk = blk0 + hb <= nIB ? hb : nIB - blk0;
+        BandInfo info;
+        info.blk0 = (int)blk0; info.nblk = (int)nblk; info.pf0 = (int)c->band_pieces.size(); info.pf1 = 0;
+        info.cstart = (int)(blk0 * JB); info.pad = 0;
+        info.joff = (long long)jrow;
+        jrow += (size_t)((nchunks - blk0 * JB) * 32 + 31) / 32 * 32;
+        int64_t start = blk0 * JB;
+        auto close_piece = [&](int64_t end) {
+            if (end > start) {
+                BandPiece pc;
+                pc.band = (int)A; pc.c0 = (int)start; pc.c1 = (int)end; pc.pad = 0;
+                c->band_pieces.push_back(pc);
+                c->band_owner.push_back((int)w);
+                start = end;
+            }
+        };
+        for (int64_t blk = blk0; blk < nIB; ++blk) {
+            const int64_t ce = (blk + 1) * JB < nchunks ? (blk + 1) * JB : nchunks;
+            const double wt = (double)chunk_weight(blk0, nblk, blk);
+            int64_t cpos = blk * JB;
+            while (cpos < ce) {
+                int64_t take = ce - cpos;
+                if (w < P - 1) {
+                    const int64_t need = (int64_t)std::ceil((next - cum) / wt);     // chunks up to the worker's boundary
+                    if (need < take) take = need < 1 ? 1 : need;
+                }
+                cum += wt * (double)take;
+                cpos += take;
+                while (w < P - 1 && cum >= next) {       // the worker's share is complete: the next one starts here
+                    close_piece(cpos);
+                    ++w;
+                    c->band_wpiece[(size_t)w] = (int)c->band_pieces.size();
+                    next = boundary(w + 1);
+                }
+            }
+        }
+        close_piece(nchunks);
+        info.pf1 = (int)c->band_pieces.size();
+        c->band_infos.push_back(info);
+    }
+    for (int64_t k = w + 1; k <= P; ++k) c->band_wpiece[(size_t)k] = (int)c->band_pieces.size();
+    lrmd::BandPart B;
+    B.N = N; B.istride = hb * IB; B.IB = (int)IB; B.nIB = (int)nIB; B.nchunks = (int)nchunks; B.nbands = (int)nbands;
+    B.hb = (int)hb; B.P = (int)P; B.wpiece = nullptr; B.pieces = nullptr; B.bands = nullptr;
+    c->bpart = B;
+    c->band_R = R;
+    c->band_jrow = jrow;
+    c->band = true;
 }
 
 void resolve(lrmd_ctx* c) {
@@ -266,16 +384,30 @@ void resolve(lrmd_ctx* c) {
         }
         c->slots = (int)smax;
         c->hmf_grid = 0;
-        resolve_sym(c, minb);
+        (void)minb;
+        resolve_band(c);
+        resolve_sym(c, !c->band);
         L.js = off; off = align_up(off + sizeof(double2) * (size_t)NJ);
         if (c->opt_precision == 1) { L.js32 = off; off = align_up(off + sizeof(float2) * ((size_t)NJ + 2)); }
         const bool two = c->model == LRMD_GRAV2D;
         const size_t rows = c->sym ? 1 : (size_t)c->slots;     // symmetric: one folded row
         L.partial0 = off; off = align_up(off + sizeof(double) * (size_t)N * rows);
         if (two) { L.partial1 = off; off = align_up(off + sizeof(double) * (size_t)N * rows); }
+        if (c->band) {
+            L.band_wpiece = off; off = align_up(off + sizeof(int) * c->band_wpiece.size());
+            L.band_pieces = off; off = align_up(off + sizeof(BandPiece) * c->band_pieces.size());
+            L.band_infos = off; off = align_up(off + sizeof(BandInfo) * c->band_infos.size());
+            const size_t irow = c->band_pieces.size() * (size_t)c->bpart.istride;
+            L.bibuf0 = off; off = align_up(off + sizeof(double) * irow);
+            if (two) { L.bibuf1 = off; off = align_up(off + sizeof(double) * irow); }
+            L.bjbuf0 = off; off = align_up(off + sizeof(double) * c->band_jrow);
+            if (two) { L.bjbuf1 = off; off = align_up(off + sizeof(double) * c->band_jrow); }
+        }
         if (c->sym) {
             L.sym_wstart = off; off = align_up(off + sizeof(int4) * c->sym_wstart.size());
             L.sym_tiles = off; off = align_up(off + sizeof(int2) * c->sym_tiles.size());
+        }
+        if (c->sym && !c->band) {
             L.ipart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots);
             if (two) { L.ipart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_slots); }
             L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows);
@@ -292,6 +424,7 @@ void resolve(lrmd_ctx* c) {
 // After resolve(): the bound workspace stays valid only if every offset is unchanged and no device-resident work table
 // (symmetric kernel) was rebuilt; otherwise the context returns to "workspace not set" (lrmd.h, lrmd_set_workspace).
 void rebind_if_changed(lrmd_ctx* c, const Layout& before, bool had_sym) {
+    // (a context that uses the band kernel also has c->sym set: the symmetric energy kernel's tables)
     if (std::memcmp(&before, &c->lay, sizeof(Layout)) != 0 || had_sym || c->sym) c->ws = nullptr;
 }
 
@@ -642,6 +775,36 @@ void pair_force_sym(Launcher& L, int upd = 0, double kickA = 0.0, double kickB =
     }
 }
 
+// Band-kernel force evaluation: one launch + the fold (which takes the update that follows, upd as above).
+void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB = 0.0, double drift = 0.0) {
+    lrmd_ctx* c = L.c;
+    double *i0 = wsd(c, c->lay.bibuf0), *i1 = wsd(c, c->lay.bibuf1), *j0 = wsd(c, c->lay.bjbuf0), *j1 = wsd(c, c->lay.bjbuf1);
+    const double pre = c->model == LRMD_RING ? -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N) : -2.0 / (double)c->N;
+    const dim3 g((unsigned)c->bpart.P), b(kBandThreads);
+    L.smem = band_smem_bytes(c->band_R);
+#define LRMD_BAND_GO(M, RR) L.go_timed(pair_force_band_kernel<M, RR>, g, b, (const double2*)js_ptr(c), c->bpart, c->eps, pre, i0, i1, j0, j1)
+    if (c->model == LRMD_RING) {
+        if (c->band_R == 8) LRMD_BAND_GO(1, 8); else LRMD_BAND_GO(1, 4);
+    } else {
+        if (c->band_R == 8) LRMD_BAND_GO(2, 8); else LRMD_BAND_GO(2, 4);
+    }
+#undef LRMD_BAND_GO
+    FusedUpdate U;
+    U.q0 = c->a0; U.q1 = nullptr; U.p0 = c->a1; U.p1 = nullptr;
+    if (c->model == LRMD_GRAV2D) { U.q1 = c->a1; U.p0 = c->a2; U.p1 = c->a3; }
+    U.kickA = kickA; U.kickB = kickB; U.drift = drift; U.js = js_ptr(c); U.js32 = js32_ptr(c);
+    const dim3 fg((unsigned)((c->N + 31) / 32)), fb(32, kFoldGroups);
+#define LRMD_BFOLD(M, UPD) \
+    L.go(pair_band_fold_kernel<M, UPD>, fg, fb, c->bpart, (const double*)i0, (const double*)i1, (const double*)j0, \
+         (const double*)j1, part0(c), part1(c), U)
+    if (c->model == LRMD_RING) {
+        if (upd == 1) LRMD_BFOLD(1, 1); else if (upd == 2) LRMD_BFOLD(1, 2); else if (upd == 3) LRMD_BFOLD(1, 3); else LRMD_BFOLD(1, 0);
+    } else {
+        if (upd == 1) LRMD_BFOLD(2, 1); else if (upd == 2) LRMD_BFOLD(2, 2); else if (upd == 3) LRMD_BFOLD(2, 3); else LRMD_BFOLD(2, 0);
+    }
+#undef LRMD_BFOLD
+}
+
 ForceRows force_rows(lrmd_ctx* c) {
     ForceRows FR;
     FR.partial0 = part0(c);
@@ -652,6 +815,7 @@ ForceRows force_rows(lrmd_ctx* c) {
 
 void pair_force(Launcher& L) {
     lrmd_ctx* c = L.c;
+    if (c->band) { pair_force_band(L); return; }
     if (c->sym) { pair_force_sym(L); return; }
     with_pair_cfg(c->pair_variant, [&](auto cfg) {
         using CFG = decltype(cfg);
@@ -700,10 +864,11 @@ int pair_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     pair_ensure_force(L);
     // A force evaluation that is one launch of the symmetric kernel takes the update that follows it into its
     // fold kernel (same arithmetic, one launch and one pass over the force row fewer per substage).
-    const bool fuse = c->sym && c->sym_batches.size() == 1 && c->opt_fuse != 0;
+    const bool fuse = (c->band || (c->sym && c->sym_batches.size() == 1)) && c->opt_fuse != 0;
     auto force_then_update = [&](bool kick2, bool drift, double kA, double kB, double d) {
         if (fuse) {
-            pair_force_sym(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
+            if (c->band) pair_force_band(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
+            else pair_force_sym(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
         } else {
             pair_force(L);
             pair_update(L, kick2, drift, kA, kB, d);
@@ -765,6 +930,22 @@ int lrmd_set_workspace(lrmd_ctx* c, void* device_ptr, size_t bytes, void* cuda_s
     if (!c || !device_ptr) return LRMD_EINVAL;
     if (bytes < c->lay.total || ((uintptr_t)device_ptr % kAlign) != 0) return LRMD_EINVAL;
     c->ws = static_cast<char*>(device_ptr);
+    if (c->band) {
+        cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+        cudaError_t e = cudaMemcpyAsync(c->ws + c->lay.band_wpiece, c->band_wpiece.data(), sizeof(int) * c->band_wpiece.size(),
+                                        cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(c->ws + c->lay.band_pieces, c->band_pieces.data(), sizeof(BandPiece) * c->band_pieces.size(),
+                                cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(c->ws + c->lay.band_infos, c->band_infos.data(), sizeof(BandInfo) * c->band_infos.size(),
+                                cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); c->ws = nullptr; return LRMD_ECUDA; }
+        c->bpart.wpiece = reinterpret_cast<const int*>(c->ws + c->lay.band_wpiece);
+        c->bpart.pieces = reinterpret_cast<const BandPiece*>(c->ws + c->lay.band_pieces);
+        c->bpart.bands = reinterpret_cast<const BandInfo*>(c->ws + c->lay.band_infos);
+    }
     if (c->sym) {
         cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
         cudaError_t e = cudaMemcpyAsync(c->ws + c->lay.sym_wstart, c->sym_wstart.data(), sizeof(int4) * c->sym_wstart.size(),
@@ -989,7 +1170,7 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             c->opt_hmf_grid = value;
             break;
         case LRMD_OPT_PAIR_SYMMETRIC:
-            if (value < -1 || value > 1) return LRMD_EINVAL;
+            if (value < -1 || value > 2) return LRMD_EINVAL;
             if (c->model == LRMD_HMF && value > 0) return LRMD_EINVAL;
             c->opt_sym = value;
             break;
@@ -1001,6 +1182,11 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
             if (value < 0 || value > (1 << 24)) return LRMD_EINVAL;
             if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
             c->opt_sym_tiles = value;
+            break;
+        case LRMD_OPT_PAIR_BAND_HEIGHT:
+            if (value < 0 || value > (1 << 20)) return LRMD_EINVAL;
+            if (c->model == LRMD_HMF && value != 0) return LRMD_EINVAL;
+            c->opt_band_height = value;
             break;
         case LRMD_OPT_PAIR_SYM_EXCHANGE:
             if (value < -1 || value > 3) return LRMD_EINVAL;
@@ -1030,13 +1216,14 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
     if (!c || !value) return LRMD_EINVAL;
     switch (key) {
         case LRMD_OPT_PAIR_PRECISION: *value = c->opt_precision; break;
-        case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : (c->sym ? c->spart.G : c->part.G); break;
+        case LRMD_OPT_PAIR_CTAS: *value = c->model == LRMD_HMF ? 0 : (c->band ? c->bpart.P : (c->sym ? c->spart.G : c->part.G)); break;
         case LRMD_OPT_HMF_VARIANT: *value = c->hmf_variant; break;
         case LRMD_OPT_PAIR_VARIANT: *value = c->pair_variant; break;
-        case LRMD_OPT_PAIR_SLOTS: *value = c->sym ? c->sym_slots : c->slots; break;
-        case LRMD_OPT_PAIR_SYMMETRIC: *value = c->sym ? 1 : 0; break;
-        case LRMD_OPT_PAIR_SYM_TILES: *value = c->sym ? c->sym_rows : 0; break;
-        case LRMD_OPT_PAIR_FUSE_UPDATE: *value = (c->sym && c->sym_batches.size() == 1 && c->opt_fuse != 0) ? 1 : 0; break;
+        case LRMD_OPT_PAIR_SLOTS: *value = c->band ? (int64_t)c->band_pieces.size() : (c->sym ? c->sym_slots : c->slots); break;
+        case LRMD_OPT_PAIR_SYMMETRIC: *value = c->band ? 2 : (c->sym ? 1 : 0); break;
+        case LRMD_OPT_PAIR_SYM_TILES: *value = (c->sym && !c->band) ? c->sym_rows : 0; break;
+        case LRMD_OPT_PAIR_BAND_HEIGHT: *value = c->band ? c->bpart.hb : 0; break;
+        case LRMD_OPT_PAIR_FUSE_UPDATE: *value = ((c->band || (c->sym && c->sym_batches.size() == 1)) && c->opt_fuse != 0) ? 1 : 0; break;
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;
@@ -1123,6 +1310,24 @@ int lrmd_pair_sym_partition(const lrmd_ctx* c, int64_t worker, int64_t* out5_hos
     out5_host[2] = st.z;                   // number of (tile, chunk) units, tile-major
     out5_host[3] = batch;                  // launch (batch of tiles) the worker belongs to
     out5_host[4] = 32 * c->sym_R;          // particles per i-tile
+    return LRMD_OK;
+}
+
+int lrmd_pair_band_partition(const lrmd_ctx* c, int64_t piece, int64_t* out8_host, int64_t* n_pieces_host) {
+    if (!c || c->model == LRMD_HMF) return LRMD_EINVAL;
+    if (n_pieces_host) *n_pieces_host = c->band ? (int64_t)c->band_pieces.size() : 0;
+    if (!out8_host) return n_pieces_host ? LRMD_OK : LRMD_EINVAL;
+    if (!c->band || piece < 0 || piece >= (int64_t)c->band_pieces.size()) return LRMD_EINVAL;
+    const BandPiece& pc = c->band_pieces[(size_t)piece];
+    const BandInfo& bi = c->band_infos[(size_t)pc.band];
+    out8_host[0] = pc.band;                          // band of the piece
+    out8_host[1] = pc.c0;                            // its columns [c0, c1), in chunks of 32 particles
+    out8_host[2] = pc.c1;
+    out8_host[3] = c->band_owner[(size_t)piece];     // worker (CTA) that owns it
+    out8_host[4] = bi.blk0;                          // the band's I-blocks blk0 .. blk0 + nblk - 1
+    out8_host[5] = bi.nblk;
+    out8_host[6] = c->bpart.IB;                      // rows per I-block = columns per J-block
+    out8_host[7] = c->bpart.P;                       // workers
     return LRMD_OK;
 }
 

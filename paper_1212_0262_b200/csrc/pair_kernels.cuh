@@ -484,18 +484,19 @@ struct SymWarpSmem {
 
 template <int MODEL, int R, bool MASK, bool DIAG>
 __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const double (&b)[R], const bool (&vi)[R],
-                                               double (&f0)[R], double (&f1)[R], SymWarpSmem& sw, int nvalid, double eps,
-                                               double onepe) {
+                                               double (&f0)[R], double (&f1)[R], const double2* __restrict__ spos,
+                                               double2* __restrict__ sg, int nvalid, double eps, double onepe) {
+    // spos / sg: the 32 slots of the packet in shared memory (positions; force sums, read and written when !DIAG)
     const int lane = threadIdx.x & 31;
-    double2 qn = sw.pos[lane];
+    double2 qn = spos[lane];
 #pragma unroll 8
     for (int s = 0; s < 32; ++s) {
         const int idx = (lane + s) & 31;
         const double2 q = qn;
-        qn = sw.pos[(idx + 1) & 31];                 // next step's position, loaded a step ahead
+        qn = spos[(idx + 1) & 31];                   // next step's position, loaded a step ahead
         double h0 = 0.0, h1 = 0.0;
         if (!DIAG) {                                 // the slot's force sum so far
-            const double2 g = sw.g[idx];
+            const double2 g = sg[idx];
             h0 = g.x;
             h1 = g.y;
         }
@@ -555,7 +556,7 @@ __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const doubl
             }
         }
         if (!DIAG) {
-            sw.g[idx] = make_double2(h0, h1);
+            sg[idx] = make_double2(h0, h1);
             __syncwarp();
         }
     }
@@ -640,11 +641,11 @@ pair_force_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, dou
             sw.g[lane] = make_double2(0.0, 0.0);
             __syncwarp();
             if (diag) {
-                if (masked) sym_chunk_smem<MODEL, R, true, true>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
-                else sym_chunk_smem<MODEL, R, false, true>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+                if (masked) sym_chunk_smem<MODEL, R, true, true>(a, b, vi, f0, f1, sw.pos, sw.g, nvalid, eps, onepe);
+                else sym_chunk_smem<MODEL, R, false, true>(a, b, vi, f0, f1, sw.pos, sw.g, nvalid, eps, onepe);
             } else {
-                if (masked) sym_chunk_smem<MODEL, R, true, false>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
-                else sym_chunk_smem<MODEL, R, false, false>(a, b, vi, f0, f1, sw, nvalid, eps, onepe);
+                if (masked) sym_chunk_smem<MODEL, R, true, false>(a, b, vi, f0, f1, sw.pos, sw.g, nvalid, eps, onepe);
+                else sym_chunk_smem<MODEL, R, false, false>(a, b, vi, f0, f1, sw.pos, sw.g, nvalid, eps, onepe);
             }
             __syncwarp();
             const double2 g = sw.g[lane];
@@ -1056,6 +1057,56 @@ struct FusedUpdate {
     float2* js32;
 };
 
+// Tail of the fold kernels, run by the thread of group 0: combines the kFoldGroups partial sums of particle i in a
+// fixed pairwise tree, writes (or adds to) the force row and applies the update UPD.
+template <int MODEL, int UPD>
+__device__ __forceinline__ void fold_finish(const double (&sf)[kFoldGroups][32], const double (&sg)[kFoldGroups][32],
+                                            long long i, bool write, double* __restrict__ out0, double* __restrict__ out1,
+                                            const FusedUpdate& U) {
+    constexpr int GR = kFoldGroups;
+    const int x = threadIdx.x;
+    double ff[GR], gg[GR];
+#pragma unroll
+    for (int m = 0; m < GR; ++m) { ff[m] = sf[m][x]; gg[m] = sg[m][x]; }
+#pragma unroll
+    for (int w = 1; w < GR; w *= 2) {      // fixed pairwise tree: (0+1), (2+3), ... then (01+23), ...
+#pragma unroll
+        for (int m = 0; m < GR; m += 2 * w) { ff[m] += ff[m + w]; gg[m] += gg[m + w]; }
+    }
+    if (write) {
+        out0[i] = ff[0];
+        if (out1) out1[i] = gg[0];
+    } else {
+        out0[i] += ff[0];
+        if (out1) out1[i] += gg[0];
+    }
+    if (UPD != 0) {     // only on single-launch evaluations: ff, gg are the whole force
+        double p = fma(U.kickA, ff[0], U.p0[i]);
+        if (UPD == 3) p = fma(U.kickB, ff[0], p);
+        U.p0[i] = p;
+        double pb = 0.0;
+        if (MODEL == 2) {
+            pb = fma(U.kickA, gg[0], U.p1[i]);
+            if (UPD == 3) pb = fma(U.kickB, gg[0], pb);
+            U.p1[i] = pb;
+        }
+        if (UPD >= 2) {
+            const double xq = fma(U.drift, p, U.q0[i]);
+            U.q0[i] = xq;
+            if (MODEL == 2) {
+                const double yq = fma(U.drift, pb, U.q1[i]);
+                U.q1[i] = yq;
+                U.js[i] = make_double2(xq, yq);
+                if (U.js32) U.js32[i] = make_float2((float)xq, (float)yq);
+            } else {
+                double sn, cs;
+                sincos_any(xq, sn, cs);
+                U.js[i] = make_double2(cs, sn);
+            }
+        }
+    }
+}
+
 template <int MODEL, int UPD>
 __global__ void __launch_bounds__(32 * kFoldGroups)
 pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double* __restrict__ ipart1,
@@ -1085,49 +1136,7 @@ pair_sym_fold_kernel(SymPart S, const double* __restrict__ ipart0, const double*
     sf[k][threadIdx.x] = f;
     sg[k][threadIdx.x] = g;
     __syncthreads();
-    if (k == 0 && i < N) {
-        const int x = threadIdx.x;
-        double ff[GR], gg[GR];
-#pragma unroll
-        for (int m = 0; m < GR; ++m) { ff[m] = sf[m][x]; gg[m] = sg[m][x]; }
-#pragma unroll
-        for (int w = 1; w < GR; w *= 2) {      // fixed pairwise tree: (0+1), (2+3), ... then (01+23), ...
-#pragma unroll
-            for (int m = 0; m < GR; m += 2 * w) { ff[m] += ff[m + w]; gg[m] += gg[m + w]; }
-        }
-        if (S.tile0 == 0) {
-            out0[i] = ff[0];
-            if (out1) out1[i] = gg[0];
-        } else {
-            out0[i] += ff[0];
-            if (out1) out1[i] += gg[0];
-        }
-        if (UPD != 0) {     // only on single-launch evaluations (tile0 = 0, tile1 = ntiles): ff, gg are the force
-            double p = fma(U.kickA, ff[0], U.p0[i]);
-            if (UPD == 3) p = fma(U.kickB, ff[0], p);
-            U.p0[i] = p;
-            double pb = 0.0;
-            if (MODEL == 2) {
-                pb = fma(U.kickA, gg[0], U.p1[i]);
-                if (UPD == 3) pb = fma(U.kickB, gg[0], pb);
-                U.p1[i] = pb;
-            }
-            if (UPD >= 2) {
-                const double x = fma(U.drift, p, U.q0[i]);
-                U.q0[i] = x;
-                if (MODEL == 2) {
-                    const double y = fma(U.drift, pb, U.q1[i]);
-                    U.q1[i] = y;
-                    U.js[i] = make_double2(x, y);
-                    if (U.js32) U.js32[i] = make_float2((float)x, (float)y);
-                } else {
-                    double sn, cs;
-                    sincos_any(x, sn, cs);
-                    U.js[i] = make_double2(cs, sn);
-                }
-            }
-        }
-    }
+    if (k == 0 && i < N) fold_finish<MODEL, UPD>(sf, sg, i, S.tile0 == 0, out0, out1, U);
 }
 
 // The partial rows of a force evaluation: [slots][N] from the ordered kernels, or the single folded row of the

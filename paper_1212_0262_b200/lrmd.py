@@ -21,6 +21,7 @@ OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 
 OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS, OPT_PAIR_SYMMETRIC, OPT_PAIR_SYM_TILES = 5, 6, 7, 8, 9
 OPT_PAIR_FUSE_UPDATE = 10
 OPT_PAIR_SYM_EXCHANGE = 11
+OPT_PAIR_BAND_HEIGHT = 12
 
 #: every symbol include/lrmd.h declares (tests check the library exports each of them)
 SYMBOLS = (
@@ -28,6 +29,7 @@ SYMBOLS = (
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
     "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard", "lrmd_pair_sym_partition", "lrmd_fp64_peak",
+    "lrmd_pair_band_partition",
 )
 
 _lib = None
@@ -81,6 +83,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_step_observe.argtypes = [_vp, _i64, _dbl, _i64, _vp, _vp]
     lib.lrmd_set_shard.argtypes = [_vp, _i64, _i64, _vp, _vp, _vp]
     lib.lrmd_pair_sym_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
+    lib.lrmd_pair_band_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
     lib.lrmd_fp64_peak.argtypes = [_int, _int, _int, _int, _int, _vp, C.c_size_t, C.POINTER(_dbl), _vp]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
@@ -217,6 +220,20 @@ def lrmd_pair_sym_partition(ctx):
         if rc != OK:
             break
         rc = load().lrmd_pair_sym_partition(ctx, w, tab[w].ctypes.data, None)
+    return rc, tab
+
+
+def lrmd_pair_band_partition(ctx):
+    """Diagnostic: (rc, table) with one row {band, c0, c1, worker, first I-block of the band, I-blocks in the band,
+    IB, workers} per piece of the band kernel's partition (an empty table if it is not in use)."""
+    import numpy as np
+    n = _i64(0)
+    rc = load().lrmd_pair_band_partition(ctx, 0, None, C.byref(n))
+    tab = np.zeros((n.value, 8), dtype=np.int64)
+    for k in range(n.value):
+        if rc != OK:
+            break
+        rc = load().lrmd_pair_band_partition(ctx, k, tab[k].ctypes.data, None)
     return rc, tab
 
 

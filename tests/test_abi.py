@@ -312,3 +312,72 @@ def test_reresolving_a_symmetric_context_unbinds_the_workspace(lrmd, how):
     assert torch.equal(th, th2) and torch.equal(p, p2)
     lrmd.lrmd_destroy(h)
     lrmd.lrmd_destroy(h2)
+
+
+@pytest.mark.parametrize("model,N,workers,height,variant", [
+    (GRAV2D, 65_536, 0, 0, -1), (GRAV2D, 1_048_576, 0, 0, -1), (RING, 100_003, 0, 0, -1), (GRAV2D, 50_000, 7, 3, 0),
+    (RING, 2049, 0, 0, 1), (GRAV2D, 33, 0, 0, -1), (GRAV2D, 300_000, 1, 0, -1), (RING, 70_001, 1000, 2, 0),
+    (GRAV2D, 4_000_000, 0, 0, -1),
+])
+def test_band_partition_covers_every_column_once_and_is_balanced(lrmd, model, N, workers, height, variant):
+    """Host logic of the band kernel (LRMD_OPT_PAIR_SYMMETRIC = 2): the pieces of a band are consecutive column ranges
+    that cover [first row of the band, N) exactly once; pieces are handed to the workers in order; the workers'
+    weights (FP64 instructions: 11 / 12 per pair above the diagonal block, 9 / 11 inside it) differ by at most one
+    chunk column of the tallest band."""
+    rc, h = lrmd.lrmd_create(model, N, 1e-3)
+    assert rc == lrmd.OK
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 2) == lrmd.OK
+    if variant >= 0:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_VARIANT, variant) == lrmd.OK
+    if workers:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, workers) == lrmd.OK
+    if height:
+        assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_BAND_HEIGHT, height) == lrmd.OK
+    rc, v = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SYMMETRIC)
+    assert rc == lrmd.OK and v == 2
+    rc, tab = lrmd.lrmd_pair_band_partition(h)
+    assert rc == lrmd.OK and len(tab) >= 1
+    IB, P = int(tab[0, 6]), int(tab[0, 7])
+    R = 4 if (variant == 0 or (variant < 0 and model == RING)) else 8
+    assert IB == 8 * 32 * R and P == (workers or 296)
+    JB = IB // 32
+    nIB, nchunks = -(-N // IB), -(-N // 32)
+    wsym, wdiag = (12, 11) if model == RING else (11, 9)
+    # bands in order, each covered once by consecutive pieces
+    band, blk_next, col = -1, 0, None
+    weights = [0] * P
+    last_worker = 0
+    for b, c0, c1, w, blk0, nblk, _, _ in (tuple(int(x) for x in row) for row in tab):
+        assert 0 <= w < P and w >= last_worker
+        last_worker = w
+        if b != band:
+            if band >= 0:
+                assert col == nchunks                  # the previous band reached the last column
+            assert b == band + 1 and blk0 == blk_next and nblk >= 1
+            band, blk_next, col = b, blk0 + nblk, blk0 * JB
+            if height:
+                assert nblk == min(height, nIB - blk0)
+        assert c0 == col and c1 > c0 and c1 <= nchunks
+        col = c1
+        for c in range(c0, c1):
+            blk = c // JB
+            weights[w] += wsym * min(max(blk - blk0, 0), nblk) + (wdiag if blk0 <= blk < blk0 + nblk else 0)
+    assert col == nchunks and blk_next == nIB
+    hb_max = max(int(r[5]) for r in tab)
+    busy = [x for x in weights if x > 0]
+    assert max(busy) - min(busy) <= 2 * (wsym * hb_max) or len(busy) < P
+    expected = 0
+    for blk0, nblk in sorted({(int(r[4]), int(r[5])) for r in tab}):
+        for blk in range(blk0, nIB):
+            nch = min((blk + 1) * JB, nchunks) - blk * JB
+            expected += (wsym * min(blk - blk0, nblk) + (wdiag if blk < blk0 + nblk else 0)) * nch
+    assert sum(weights) == expected
+    rc, nbytes = lrmd.lrmd_workspace_bytes(h)
+    assert rc == lrmd.OK
+    if N == 1_048_576:
+        assert nbytes < 1_000_000_000          # one launch per force evaluation on < 1 GB of scratch (was 3.56 GB, 128 launches)
+    lrmd.lrmd_destroy(h)
+    rc, h = lrmd.lrmd_create(model, 4096, 1e-3)          # below 49,152 the warp-level kernel is the default: empty table
+    rc, tab = lrmd.lrmd_pair_band_partition(h)
+    assert rc == lrmd.OK and len(tab) == 0
+    lrmd.lrmd_destroy(h)

@@ -1,0 +1,124 @@
+"""Parity of the band kernel (LRMD_OPT_PAIR_SYMMETRIC = 2, csrc/band_kernels.cuh: Newton's third law with both
+sides' sums kept on chip, SURVEY.md 8(f) N4 / PAPER.md:108) with the oracle, through the C ABI, on the same seeded
+inputs and at BASELINE.json's tolerances (forces 1e-12 A_i, trajectory 1e-9 after 10 steps)."""
+import math
+
+import numpy as np
+import pytest
+
+from test_gpu_parity import FTOL, GRAV2D, RING, XTOL, _check_forces, _eps, _p, _q, _state, torch  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def _forces(lrmd, model, N, eps, st, opts):
+    ctx = lrmd.Context(model, N, eps, options=opts)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    ctx.set_state(*st)
+    f = ctx.forces()
+    got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    ctx.close()
+    return got
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N", [1, 2, 31, 33, 257, 1000, 1024, 1025, 2047, 2049, 4099, 10_007, 20_011])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_band_force_kernel_matches_oracle(lrmd, ref, torch, model, N, variant):
+    """I-blocks of 1024 (variant 0) or 2048 (variant 1) rows: one block, several blocks, ragged last tile, last chunk
+    and last block; any number of workers (pieces shorter than 8 chunks, workers without work) and band heights."""
+    eps = _eps(model)
+    st = _state(model, N, 7000 + N)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=0)
+    for workers, height in ((0, 0), (1, 0), (5, 1), (37, 2), (1000, 3)):
+        opts = {lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_VARIANT: variant, lrmd.OPT_PAIR_CTAS: workers,
+                lrmd.OPT_PAIR_BAND_HEIGHT: height}
+        got = _forces(lrmd, model, N, eps, st, opts)
+        _check_forces(model, got, (f0, f1), (A0, A1))
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+def test_band_kernel_default_shape_several_bands(lrmd, ref, torch, model):
+    """N = 70,001: beyond the default switch (49,152), 35 (2D) / 69 (Ring) I-blocks, default band height and workers;
+    forces on sampled rows against the oracle (each against all N)."""
+    eps = _eps(model)
+    N = 70_001
+    st = _state(model, N, 71)
+    q0, q1 = _q(model, st)
+    ctx = lrmd.Context(model, N, eps)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    ctx.set_state(*st)
+    f = ctx.forces()
+    got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    ctx.close()
+    rows = np.unique(np.concatenate([np.arange(0, 300), np.arange(N - 300, N),
+                                     np.random.default_rng(5).choice(N, 3000, replace=False)]))
+    r0, r1, A0, A1 = ref.forces_rows(model, eps, q0, q1, rows, form=0, with_abs=True)
+    _check_forces(model, tuple(None if g is None else g[rows] for g in got), (r0, r1), (A0, A1))
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+def test_band_kernel_trajectory_momentum_and_reproducibility(lrmd, ref, torch, model):
+    eps = _eps(model)
+    N = 6007
+    st = _state(model, N, 89)
+    outs = []
+    for _ in range(2):
+        ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_BAND_HEIGHT: 2})
+        ctx.set_state(*st)
+        ctx.step(10, 0.01)
+        outs.append(ctx.state_numpy())
+        ctx.close()
+    for x, y in zip(*outs):
+        assert np.array_equal(x, y)          # fixed order of every sum: bitwise reproducible
+    r = [a.copy() for a in st]
+    q0, q1 = _q(model, r)
+    p0, p1 = _p(model, r)
+    ref.step(model, eps, q0, q1, p0, p1, 10, 0.01, form=1)
+    for g, w in zip(outs[0], r):
+        assert np.max(np.abs(g - w)) <= XTOL
+    pk = (2, 3) if model == GRAV2D else (1,)
+    for k in pk:     # antisymmetric pair forces: total momentum conserved to rounding
+        assert abs(math.fsum(outs[0][k]) - math.fsum(st[k])) <= 1e-13 * math.fsum(np.abs(st[k]))
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+def test_band_update_fused_into_fold_is_bit_identical(lrmd, torch, model):
+    eps = _eps(model)
+    N = 5003
+    st = _state(model, N, 322)
+    res = []
+    for fuse, single in ((1, False), (0, False), (1, True)):
+        ctx = lrmd.Context(model, N, eps, options={lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_FUSE_UPDATE: fuse})
+        assert ctx.get_option(lrmd.OPT_PAIR_FUSE_UPDATE) == fuse
+        ctx.set_state(*st)
+        if single:
+            for _ in range(5):
+                ctx.step(1, 0.01)
+        else:
+            ctx.step(5, 0.01)
+        f = ctx.forces()
+        f = [t.cpu().numpy() for t in f] if model == GRAV2D else [f.cpu().numpy()]
+        res.append(list(ctx.state_numpy()) + f + [ctx.energy().cpu().numpy()])
+        ctx.close()
+    for other in res[1:]:
+        for x, y in zip(res[0], other):
+            assert np.array_equal(x, y)
+
+
+def test_band_kernel_agrees_with_the_other_pair_kernels(lrmd, torch):
+    """Same state, three kernels (ordered, warp-level symmetric, band): forces agree to rounding of the sums."""
+    N = 9001
+    st = _state(GRAV2D, N, 17)
+    fs = []
+    for sym in (0, 1, 2):
+        ctx = lrmd.Context(GRAV2D, N, 1e-3, options={lrmd.OPT_PAIR_SYMMETRIC: sym})
+        assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == sym
+        ctx.set_state(*st)
+        fs.append([t.cpu().numpy() for t in ctx.forces()])
+        ctx.close()
+    scale = max(np.abs(fs[0][0]).max(), np.abs(fs[0][1]).max())
+    for other in fs[1:]:
+        for a, b in zip(fs[0], other):
+            assert np.max(np.abs(a - b)) <= 1e-11 * scale

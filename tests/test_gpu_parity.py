@@ -588,12 +588,17 @@ def test_symmetric_default_choice(lrmd, torch):
     c = lrmd.Context(GRAV2D, 1_048_576, 1e-3)
     d = lrmd.Context(GRAV2D, 65_536, 1e-3, options={lrmd.OPT_PAIR_SYMMETRIC: 0})
     e = lrmd.Context(GRAV2D, 1000, 1e-3)
-    assert a.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and b.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
-    assert b.get_option(lrmd.OPT_PAIR_SYM_TILES) == 256     # all 256 tiles in one launch (268 MB of j-side rows)
-    assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and c.get_option(lrmd.OPT_PAIR_SYM_TILES) == 64   # 64 launches of 64 tiles
+    b1 = lrmd.Context(GRAV2D, 65_536, 1e-3, options={lrmd.OPT_PAIR_SYMMETRIC: 1})
+    c1 = lrmd.Context(GRAV2D, 1_048_576, 1e-3, options={lrmd.OPT_PAIR_PRECISION: 1})
+    # 2048 <= N < 49,152: warp-level symmetric kernel; beyond: band kernel (one launch, any N)
+    assert a.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and b.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2 and c.get_option(lrmd.OPT_PAIR_FUSE_UPDATE) == 1
+    assert b1.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
+    assert b1.get_option(lrmd.OPT_PAIR_SYM_TILES) == 256    # all 256 tiles in one launch (268 MB of j-side rows)
+    # fp32 pair arithmetic has no band kernel: warp-level kernel, 64 launches of 64 tiles at N = 2^20
+    assert c1.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and c1.get_option(lrmd.OPT_PAIR_SYM_TILES) == 64
     assert d.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0 and e.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0
-    e.close()
-    for x in (a, b, c, d):
+    for x in (a, b, c, d, e, b1, c1):
         x.close()
 
 
