@@ -1,14 +1,16 @@
 #!/usr/bin/env python
 """bench.py — throughput of the lrmd hot path on B200, one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload KEY] [--only] [--f32-pairs] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload KEY] [--only] [--f32-pairs] [--ordered-pairs]
+                    [--sharded] [--fp64-peak] [--impl reference]
 
 A bench "step" is one complete integrator time step of the workload (three force
 evaluations + the kick/drift updates — what the paper's Tables 1-3 time).  The primary workload is
-BASELINE.json configs[1] (Ring, N = 16,384, eps = 0.01, dt = 0.01); with one GPU and without --only
-the other single-GPU configs are measured too and reported under "others" in the same line, together
-with the ordered-pair kernels (the paper's own scheme, LRMD_OPT_PAIR_SYMMETRIC = 0) on the pair configs
-and config 5's fp32-pair variant.
+BASELINE.json configs[4], the largest single-GPU configuration (2D self-gravitating, N = 1,048,576,
+eps = 1e-3, dt = 0.005, fp64); with one GPU and without --only the other configs are measured too and
+reported under "others" in the same line, together with the ordered-pair kernels (the paper's own
+scheme, LRMD_OPT_PAIR_SYMMETRIC = 0) on the pair configs, config 5's fp32-pair variant and the HMF
+sizes of the paper's Table 1.
 
 Numbers reported (all measured in this process, never under a profiler):
   value      whole-job throughput, state resident in HBM, CUDA events on the launching stream
@@ -55,17 +57,28 @@ SYM_PAIR_FLOP = {1: 10.0, 2: 10.0}
 SYM_PAIR_FP64_INSTR = {1: 6.0, 2: 5.5}
 HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` captures (profiles/r01d_summary.md names the commands); None = not captured.
-# hmf_5e7: 800.0 MB read + 741.7 MB written of 1600 MB algorithmic (the last lines written are still in L2
-# when the kernel ends); the pair kernels read the 16 N (8 N for fp32) byte j-stream once from DRAM, the
-# tiles' re-reads hit L2.
-NCU_TRAFFIC_BYTES = {"ring_16k": 279808.0, "grav2d_64k": 1067264.0, "hmf_5e7": 1541759232.0, "grav2d_1m": None,
-                     "hmf_1e4": None, "grav2d_64k_f32": 554240.0,
-                     # symmetric kernel (profiles/r01f_summary.md): j-stream reads + the j-side rows it writes
-                     "ring_16k_sym": 404480.0, "grav2d_64k_sym": 98298368.0, "grav2d_64k_f32_sym": 95257600.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel come from the committed
+# `ncu --set full` captures: profiles/r02_traffic.csv names, per bench entry, the kernel, the two byte counts and
+# the capture they were read from (profiles/r02_summary.md gives the commands).
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
 
-DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5}
+
+def ncu_traffic(entry, kernel):
+    """(bytes per launch, source) of `kernel` in bench entry `entry` from profiles/r02_traffic.csv, or (None, why)."""
+    import csv
+    if not os.path.exists(TRAFFIC_CSV):
+        return None, "profiles/r02_traffic.csv missing"
+    with open(TRAFFIC_CSV) as fh:
+        for row in csv.DictReader(fh):
+            if row["entry"] == entry:
+                if row["kernel"] != kernel:
+                    return None, "capture is of %s, this run launched %s" % (row["kernel"], kernel)
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), "profiles/" + row["capture"]
+    return None, "no capture of this entry"
+
+
+DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5,
+                 "hmf_1e5": 1000, "hmf_1e6": 500, "hmf_1e7": 200}
 
 
 def measured_peaks():
@@ -158,7 +171,7 @@ def units_per_force(w):
 
 
 def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False, ordered_pairs=False,
-                 force_symmetric=False):
+                 force_symmetric=False, roofline_steps=2000, e2e_steps=20, fp64_peak=None):
     import torch
     from paper_1212_0262_b200 import lrmd
 
@@ -227,9 +240,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     out = {
         "metric": metric, "value": value, "unit": unit, "ms_per_step": ms_max / K,
         "gpu_launches": int(launches), "clocks": clocks,
-        "l2": ("inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)) if larger_than_l2 else
-              ("not flushed: %.2f MB working set is on-chip by design, latency-bound case" % (state_bytes / 1e6)
-               if resident_by_design else "L2 flushed (256 MiB write) before every timed step"),
+        "l2": l2_statement(w),
         "options": {"pair_ctas": ctx.get_option(lrmd.OPT_PAIR_CTAS), "pair_variant": ctx.get_option(lrmd.OPT_PAIR_VARIANT),
                     "pair_slots": ctx.get_option(lrmd.OPT_PAIR_SLOTS), "graph": ctx.get_option(lrmd.OPT_GRAPH),
                     "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT),
@@ -240,18 +251,21 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     # ---- roofline of the dominant kernel: second pass with an event pair around each of its launches
     if with_roofline:
         ctx.set_option(lrmd.OPT_KERNEL_TIMING, 1)
-        Kr = min(K, 2000)
+        Kr = min(K, roofline_steps)
         ctx.kernel_time()
         ms_r = timed_pass(Kr)
         kms, kn = ctx.kernel_time()
         ctx.set_option(lrmd.OPT_KERNEL_TIMING, 0)
         avg_s = (kms / max(kn, 1)) * 1e-3
         if w.model != 0:
-            # pair models: per FORCE EVALUATION (3 per step; the symmetric kernel may take several launches, one per
-            # batch of i-tiles, for one evaluation)
+            # pair models: per FORCE EVALUATION (3 per step; the warp-level symmetric kernel may take several launches, one
+            # per batch of i-tiles, for one evaluation)
             avg_s = (kms / (3.0 * Kr)) * 1e-3
         clk = (clocks.get("sm_mhz") or peaks["sm_max_mhz"])
+        symk = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) if w.model != 0 else 0     # 0 ordered, 1 warp-level, 2 band
         if w.model == 0:
+            kernel = {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT),
+                                                                             "hmf_substage_tma_kernel")
             bytes_per_launch = HMF_BYTES_PER_PARTICLE_SUBSTAGE * w.N
             if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3:
                 # cluster-resident kernel: one launch runs all Kr steps with the state in registers; the figure is
@@ -261,45 +275,62 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
             roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
                     "algorithmic_bytes_per_launch": bytes_per_launch}
+            if 2.0 * state_bytes <= L2_BYTES:
+                roof["note"] = ("state (%.1f MB) fits the 126 MB L2: the substages stream it through L2, not HBM; the HBM figure "
+                                "is context only" % (state_bytes / 1e6))
         elif f32_pairs:
             # fp32 pair arithmetic: one MUFU.RCP per pair on the special-function unit, 16 lanes per SM per clock
-            sym = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
-            mufu = float(w.N) * float(w.N) * (0.5 if sym else 1.0)      # executed: one per (un)ordered pair evaluated
+            kernel = "grav_force_sym_f32_kernel" if symk else "grav_force_f32_kernel"
+            mufu = float(w.N) * float(w.N) * (0.5 if symk else 1.0)      # executed: one per (un)ordered pair evaluated
             peak = SM_COUNT * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
             achieved = mufu / avg_s / 1e12
             roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T MUFU.RCP/s",
                     "frac": achieved / peak,
                     "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: 6 FADD/FFMA per pair",
                     "algorithmic_mufu_per_launch": mufu}
-            if sym:
+            if symk:
                 roof["note"] = ("symmetric fp32 kernel: one MUFU.RCP and 8 FADD/FFMA per UNORDERED pair (N^2/2 evaluations deliver "
                                 "N^2 pair interactions), ~10.5 issued instructions per evaluation: instruction issue binds before "
                                 "the SFU; by the ordered-pair convention (one MUFU per delivered pair) the launch reads %.3f"
                                 % (float(w.N) * float(w.N) / avg_s / 1e12 / peak))
         else:
-            sym = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
-            flop = (SYM_PAIR_FLOP if sym else PAIR_FLOP)[w.model] * w.N * w.N
+            kernel = {0: "pair_force_kernel", 1: "pair_force_sym_kernel", 2: "pair_force_band_kernel"}[symk]
+            flop = (SYM_PAIR_FLOP if symk else PAIR_FLOP)[w.model] * w.N * w.N
             achieved = flop / avg_s / 1e12
             peak = SM_COUNT * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-            instr_rate = (SYM_PAIR_FP64_INSTR if sym else PAIR_FP64_INSTR)[w.model] * w.N * w.N / avg_s
+            instr_rate = (SYM_PAIR_FP64_INSTR if symk else PAIR_FP64_INSTR)[w.model] * w.N * w.N / avg_s
             roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                     "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",
                     "algorithmic_flop_per_launch": flop,
                     "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
                     "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
-            if sym:
+            if fp64_peak is not None:
+                # the committed microbenchmark (lrmd_fp64_peak): what the FP64 pipe sustains on this box
+                roof["peak_measured"] = fp64_peak["dfma_tflops"]
+                roof["frac_of_peak_measured"] = achieved / fp64_peak["dfma_tflops"]
+                roof["peak_measured_what"] = fp64_peak["what"]
+                roof["fp64_pipe_frac_of_measured_issue_rate"] = instr_rate / fp64_peak["dmul_instr_per_s"]
+            if symk:
                 roof["note"] = ("symmetric kernel: every unordered pair evaluated once (N^2/2 evaluations deliver N^2 pair "
                                 "interactions); flops and instructions are the EXECUTED ones; by the ordered-pair convention "
                                 "(%g flop per delivered pair) the same launch reads %.3f of peak"
                                 % (PAIR_FLOP[w.model], PAIR_FLOP[w.model] * w.N * w.N / avg_s / 1e12 / peak))
-        roof.update({"kernel": {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel") if w.model == 0 else (("grav_force_sym_f32_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "grav_force_f32_kernel") if f32_pairs else
-                                 ("pair_force_sym_kernel" if ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 else "pair_force_kernel")),
-                     "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
-                     "kernel_launches_per_force_evaluation": (kn / (3.0 * Kr)) if w.model != 0 else None,
+        entry = w.key + ("_f32pairs" if f32_pairs else "") + ("_ordered_pairs" if (w.model != 0 and not symk) else "")
+        traffic, tsrc = ncu_traffic(entry, kernel)
+        if w.model == 0:
+            alg_bytes = roof["algorithmic_bytes_per_launch"]
+        else:
+            # the j-stream read once (16 N, fp32 stream 8 N) + the force written once (8 N per component)
+            alg_bytes = (8.0 if f32_pairs else 16.0) * w.N + 8.0 * w.N * (2 if w.model == 2 else 1)
+        launches_per_eval = (kn / (3.0 * Kr)) if w.model != 0 else None
+        roof.update({"kernel": kernel, "kernel_avg_ms": avg_s * 1e3, "kernel_launches_timed": kn,
+                     "kernel_launches_per_force_evaluation": launches_per_eval,
                      "kernel_share_of_step": kms / ms_r if ms_r > 0 else None,
-                     "traffic": NCU_TRAFFIC_BYTES.get(w.key + ("_f32" if f32_pairs else "") +
-                                                      ("_sym" if (w.model != 0 and
-                                                                  ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1) else ""))})
+                     "traffic": traffic, "traffic_source": tsrc,
+                     "traffic_what": "dram__bytes_read.sum + dram__bytes_write.sum per launch (ncu --set full)",
+                     "algorithmic_dram_bytes_per_force_evaluation" if w.model != 0 else "algorithmic_dram_bytes_per_launch": alg_bytes,
+                     "traffic_ratio": (traffic * (launches_per_eval or 1.0) / alg_bytes) if traffic is not None else None,
+                     "workspace_bytes": ctx.workspace_bytes()})
         out["roofline"] = roof
 
     # ---- energy sums (rows a-E1..a-E3), timed apart from the steps
@@ -324,7 +355,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     # ---- end to end through lrmd_step_host: pinned host buffers, copies inside the timed region
     if with_e2e:
         host = [torch.from_numpy(a.copy()).pin_memory() for a in st]
-        Ke = max(1, min(K, 20 if w.model != 0 else K))
+        Ke = max(1, min(K, e2e_steps if w.model != 0 else K))
         ctx.step_host(host, 1, w.dt)                          # warm-up of the copy path
         for h, a in zip(host, st):
             h.copy_(torch.from_numpy(a))
@@ -386,6 +417,25 @@ def oracle_sample_rate(w, seconds, nthreads=0):
     return R * w.N / el, f"forces on {R} sampled rows x all {w.N} j ({what}), OpenMP over rows", threads
 
 
+def l2_statement(w):
+    """How the timed iterations keep L2 from flattering the number (the same for every arm of a workload)."""
+    narr = 4 if w.model == 2 else 2
+    state_bytes = narr * w.N * 8
+    if state_bytes > L2_BYTES:
+        return "inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)
+    if w.key == "hmf_1e4":
+        return "not flushed: %.2f MB working set is on-chip by design, latency-bound case" % (state_bytes / 1e6)
+    return "L2 flushed (256 MiB write) before every timed step"
+
+
+def workload_config(w, world):
+    """The `config` object of the JSON line: the workload, identical for the b200 and the reference arm."""
+    return {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt,
+            "step": "one 4th-order time step = 3 force evaluations + kick/drift updates (PAPER.md:54-63)",
+            "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
+            "l2": l2_statement(w)}
+
+
 def run_reference(args, w):
     """--impl reference: the oracle timed on the host cores; each step is a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -404,7 +454,7 @@ def run_reference(args, w):
         "impl": "reference", "metric": metric, "value": value, "unit": unit, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": None, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt},
+        "config": workload_config(w, int(os.environ.get("WORLD_SIZE", "1"))),
         "cpu_baseline": {"value": value, "unit": unit, "cores": threads, "kind": "oracle", "sample": "per step: " + desc},
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -452,17 +502,100 @@ def fp64_peak_table(device=None, iters=20000, full=True):
     return res
 
 
+# ---- strong scaling through the sharded path — opt-in, never the default ------
+
+def sharded_plan(w, world, rank):
+    """Host logic of --sharded: which particles rank `rank` owns and what one substage exchanges.
+    HMF: one all-reduce of 2 doubles; Ring / 2D: one all-gather of the packed positions, 16 bytes per
+    particle.  Pure host code (tested with gloo, world 2)."""
+    from paper_1212_0262_b200 import sharded
+    i0, n = sharded.shard_bounds(w.N, world)[rank]
+    if w.model == 0:
+        exchange = {"collective": "all_reduce", "bytes_per_substage": 16}
+        units_per_step = float(w.N)
+    else:
+        exchange = {"collective": "all_gather", "bytes_per_substage": 16 * w.N}
+        units_per_step = 3.0 * float(w.N) * float(w.N)
+    return {"i0": i0, "n_local": n, "exchange": exchange, "units_per_step": units_per_step,
+            "rows_x_columns": [n, w.N] if w.model != 0 else None}
+
+
+def strong_scaling_value(units_per_step, steps, ms_max):
+    """Whole-job throughput of ONE problem split over the ranks: its units / the slowest rank's device time."""
+    return units_per_step * steps / (ms_max * 1e-3)
+
+
+def run_sharded(w, K, W, dist_ctx, world, rank):
+    import torch
+    from paper_1212_0262_b200 import sharded
+    dev = torch.device("cuda", torch.cuda.current_device())
+    plan = sharded_plan(w, world, rank)
+    coll = sharded.TorchDistCollectives(dist_ctx, rank, world) if dist_ctx is not None else sharded.SingleRankCollectives()
+    ctx = sharded.ShardedContext(w.model, w.N, w.eps, coll, device=dev)
+    ctx.set_state_global(*w.state())
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if dist_ctx is not None:
+            dist_ctx.barrier()
+        torch.cuda.synchronize(dev)
+
+    ctx.step(W, w.dt)
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device()).start()
+    l0 = ctx.launch_count()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    ctx.step(K, w.dt)
+    b.record(stream)
+    b.synchronize()
+    ms = a.elapsed_time(b)
+    launches = ctx.launch_count() - l0
+    barrier()
+    clocks = sampler.stop()
+    ms_max = max_over_ranks(ms, dist_ctx, dev)
+    metric, unit, _ = units_per_force(w)
+    ctx.close()
+    return {"metric": metric, "value": strong_scaling_value(plan["units_per_step"], K, ms_max), "unit": unit, "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(workload_config(w, world), parallelism="sharded: %d ranks, rows split, %s of %d bytes per substage"
+                           % (world, plan["exchange"]["collective"], plan["exchange"]["bytes_per_substage"])),
+            "clocks": clocks, "e2e": None, "gpu_launches": int(launches),
+            "note": "opt-in strong-scaling line (lrmd_set_shard + torch.distributed collectives between the kernels); "
+                    "BASELINE.json's north_star fixes one GPU, so the default bench line runs replicas"}
+
+
+def fp64_peak_summary():
+    """The numbers bench.py quotes beside the derived FP64 peak: sustained DFMA rate (two operands shared, the best
+    case the register file allows), DMUL rate (two register operands: the pipe's issue rate) and the rate of a DFMA
+    that reads three private registers (what an accumulate fma(dx, y, f) of the pair kernels is), 32 warps per SM."""
+    t = fp64_peak_table(full=False)
+    ops = t["ops"]
+    dfma, dmul, dfma3 = ops["dfma"]["32"], ops["dmul"]["32"], ops["dfma_3_private_regs"]["32"]
+    return {"dfma_tflops": 2.0 * dfma["instr_per_s"] / 1e12, "dfma_instr_per_s": dfma["instr_per_s"],
+            "dmul_instr_per_s": dmul["instr_per_s"], "dfma_3_private_regs_instr_per_s": dfma3["instr_per_s"],
+            "sm_mhz": dfma["sm_mhz"],
+            "what": "lrmd_fp64_peak (bench.py --fp64-peak), 32 warps per SM: DFMA a*m+c %.3e instr/s = %.2f TFLOP/s, DMUL %.3e "
+                    "instr/s, DFMA on three private registers %.3e instr/s, SM clock held %.0f MHz"
+                    % (dfma["instr_per_s"], 2.0 * dfma["instr_per_s"] / 1e12, dmul["instr_per_s"], dfma3["instr_per_s"],
+                       dfma["sm_mhz"])}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--workload", default="ring_16k")
+    ap.add_argument("--workload", default="grav2d_1m")
     ap.add_argument("--only", action="store_true", help="primary workload only (no 'others', no cpu_baseline)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--f32-pairs", action="store_true", help="GRAV2D workloads: fp32 pair arithmetic (PAPER.md:110)")
     ap.add_argument("--fp64-peak", action="store_true", help="run only the FP64 issue-rate microbenchmark and print its table")
+    ap.add_argument("--ordered-pairs", action="store_true", help="pair workloads: the paper's scheme, every ordered pair (PAPER.md:108)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="strong scaling through ShardedContext (lrmd_set_shard + NCCL collectives) instead of replicas")
     args = ap.parse_args()
 
     if args.fp64_peak:
@@ -475,7 +608,8 @@ def main():
         return 0
 
     from paper_1212_0262_b200 import inputs
-    w = inputs.WORKLOADS[args.workload]
+    all_workloads = dict(inputs.WORKLOADS, **inputs.TABLE1_WORKLOADS)
+    w = all_workloads[args.workload]
     if args.impl == "reference":
         args.steps = args.steps or 3
         args.warmup = 1 if args.warmup is None else args.warmup
@@ -497,52 +631,66 @@ def main():
     dist_ctx = None
     if world > 1:
         import torch.distributed as dist
+        if args.sharded:
+            os.environ.setdefault("NCCL_DEBUG", "INFO")     # the communicator's rank count shows in the log
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         dist_ctx = dist
 
-    res = run_workload(w, K, W, dist_ctx, f32_pairs=bool(args.f32_pairs and w.model == 2))
+    if args.sharded:
+        line = run_sharded(w, K, W, dist_ctx, world, rank)
+        if rank == 0:
+            print(json.dumps(line))
+        if dist_ctx is not None:
+            dist_ctx.barrier()
+            dist_ctx.destroy_process_group()
+        return 0
+
+    f32 = bool(args.f32_pairs and w.model == 2)
+    peak = fp64_peak_summary() if (w.model != 0 and not f32) else None
+    # the roofline pass and the end-to-end call repeat the steps: bounded for the seconds-long steps of config 5
+    heavy = w.key == "grav2d_1m"
+    res = run_workload(w, K, W, dist_ctx, f32_pairs=f32, ordered_pairs=bool(args.ordered_pairs and w.model != 0),
+                       roofline_steps=(3 if heavy else 2000), e2e_steps=(2 if heavy else 20), fp64_peak=peak)
     line = {
         "metric": res["metric"], "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if (args.f32_pairs and w.model == 2) else "f64", "data": "synthetic",
-        "config": {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt,
-                   "step": "one 4th-order time step = 3 force evaluations + kick/drift updates (PAPER.md:54-63)",
-                   "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
-                   "l2": res["l2"], "options": res["options"]},
+        "dtype": "f32" if f32 else "f64", "data": "synthetic",
+        "config": workload_config(w, world), "options": res["options"],
         "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
         "roofline": res.get("roofline"), "energy": res.get("energy"),
     }
 
+    keep = ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options", "clocks", "roofline", "e2e", "energy")
     if world == 1 and not args.only:
         others = {}
-        for key in ("grav2d_64k", "hmf_5e7", "grav2d_1m", "hmf_1e4"):
+
+        def add(name, ow, steps, **kw):
+            r = run_workload(ow, steps, 3, None, fp64_peak=peak, **kw)
+            others[name] = {k: r[k] for k in keep if k in r}
+            others[name]["steps"] = steps
+
+        for key in ("ring_16k", "grav2d_64k", "hmf_5e7", "grav2d_1m", "hmf_1e4"):
             if key == w.key:
                 continue
-            ow = inputs.WORKLOADS[key]
-            r = run_workload(ow, DEFAULT_STEPS[key], 3, None, with_e2e=(key != "grav2d_1m"))
-            others[key] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options",
-                                              "clocks", "roofline", "e2e", "energy") if k in r}
-            others[key]["steps"] = DEFAULT_STEPS[key]
-        # the paper's own scheme, every ORDERED pair, on the configs where the symmetric kernel is the default
+            add(key, inputs.WORKLOADS[key], DEFAULT_STEPS[key], with_e2e=(key != "grav2d_1m"), roofline_steps=(3 if key == "grav2d_1m" else 2000))
+        # HMF at the sizes of the paper's Table 1 that lie between configs 1 and 4
+        for key, ow in inputs.TABLE1_WORKLOADS.items():
+            if key != w.key:
+                add(key, ow, DEFAULT_STEPS[key], with_e2e=False)
+        # the paper's own scheme, every ORDERED pair, on the configs where a symmetric kernel is the default
         for key in ("ring_16k", "grav2d_64k", "grav2d_1m"):
-            ow = inputs.WORKLOADS[key]
-            r = run_workload(ow, 3 if key == "grav2d_1m" else DEFAULT_STEPS[key], 3, None, with_e2e=False, ordered_pairs=True)
-            others[key + "_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
-                                                                 "options", "clocks", "roofline") if k in r}
-            others[key + "_ordered_pairs"]["steps"] = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]
+            steps = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]
+            add(key + "_ordered_pairs", inputs.WORKLOADS[key], steps, with_e2e=False, ordered_pairs=True, roofline_steps=3 if key == "grav2d_1m" else 2000)
         # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
-        r = run_workload(inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], 3, None, with_e2e=False, f32_pairs=True)
-        others["grav2d_1m_f32pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2",
-                                                           "options", "clocks", "roofline") if k in r}
-        others["grav2d_1m_f32pairs"]["steps"] = DEFAULT_STEPS["grav2d_1m"]
+        add("grav2d_1m_f32pairs", inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], with_e2e=False, f32_pairs=True, roofline_steps=3)
         others["grav2d_1m_f32pairs"]["dtype"] = "f32 pair terms, f64 state and accumulation"
-        r = run_workload(inputs.WORKLOADS["grav2d_1m"], 3, 3, None, with_e2e=False, f32_pairs=True, ordered_pairs=True)
-        others["grav2d_1m_f32pairs_ordered_pairs"] = {k: r[k] for k in ("metric", "value", "unit", "ms_per_step", "gpu_launches",
-                                                                         "l2", "options", "clocks", "roofline") if k in r}
-        others["grav2d_1m_f32pairs_ordered_pairs"]["steps"] = 3
+        add("grav2d_1m_f32pairs_ordered_pairs", inputs.WORKLOADS["grav2d_1m"], 3, with_e2e=False, f32_pairs=True, ordered_pairs=True,
+            roofline_steps=3)
         line["others"] = others
         rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
-        line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc}
+        line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc,
+                                "note": "the oracle is an unoptimised checker (compensated sums, true division, -O2 without "
+                                        "contraction), not a tuned CPU code: a reported baseline, not a speedup claim"}
 
     if rank == 0:
         print(json.dumps(line))

@@ -59,8 +59,11 @@ enum {
 
 /* lrmd_set_option keys */
 enum {
-    LRMD_OPT_PAIR_PRECISION = 0, /* 0 = fp64 pair arithmetic (default); 1 = fp32 pair arithmetic with
-                                    chunked fp32 -> fp64 accumulation (GRAV2D only)      */
+    LRMD_OPT_PAIR_PRECISION = 0, /* 0 = fp64 pair arithmetic (default); 1 = fp32 pair arithmetic with chunked
+                                    fp32 -> fp64 accumulation: GRAV2D on positions rounded to
+                                    fp32, RING on (cos, sin)(theta / 2) rounded to fp32 (half-angle form: eq.(9)'s
+                                    denominator cancels to ~eps and would lose the 1e-5 tolerance in fp32); needs
+                                    eps >= 1e-30; HMF: LRMD_EUNSUPPORTED                                            */
     LRMD_OPT_PAIR_CTAS = 1,      /* pair models: number of CTAs G the flattened (i-tile, j) space is divided
                                     into, equal shares (0 = choose from N: 148 x resident CTAs x waves)  */
     LRMD_OPT_GRAPH = 2,          /* 1 = lrmd_step replays a captured CUDA graph of one step (default
@@ -111,6 +114,10 @@ int lrmd_destroy(lrmd_ctx* ctx);
  * (256-byte aligned), then bind it.  Changing an option that alters the size returns the
  * context to "workspace not set".  The contents are private to the library. */
 int lrmd_workspace_bytes(const lrmd_ctx* ctx, size_t* bytes);
+/* lrmd_set_workspace copies the small work tables of the symmetric / band pair kernels (a few KB to a few MB, built on
+ * the host when the options were resolved) into the workspace with cudaMemcpyAsync on cuda_stream and SYNCHRONISES
+ * that stream before returning (the host tables may be rebuilt by the next lrmd_set_option).  For the other contexts
+ * (HMF, ordered pair kernels) it touches no device memory and does not synchronise. */
 int lrmd_set_workspace(lrmd_ctx* ctx, void* device_ptr, size_t bytes, void* cuda_stream);
 
 /* Bind the state arrays, updated IN PLACE by lrmd_step.

@@ -54,10 +54,15 @@ struct BandPart {
 // dynamic shared memory: positions and force sums of one J-block + one mbarrier
 constexpr size_t band_smem_bytes(int R) { return (size_t)2 * kBandWarps * 32 * R * sizeof(double2) + 16; }
 
-template <int MODEL, int R>
+// WITHV: the launch also delivers the potential energy (rows a-E2 / a-E3 fused into the force kernel: "compute any
+// properties of interest" every step, listing step 12): vband[CTA] = pre_v * (the CTA's pairs' terms,
+// log(r^2 + eps) or d^(-1/2)); a block's own pairs are met twice and j = i once by the DIAG walk: halved, and the
+// self terms (exactly log eps; for Ring the value the same arithmetic gives) removed again.
+template <int MODEL, int R, bool WITHV>
 __global__ void __launch_bounds__(kBandThreads, 2)
 pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, double pre, double* __restrict__ ibuf0,
-                       double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1) {
+                       double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1, double pre_v,
+                       double* __restrict__ vband) {
     extern __shared__ __align__(128) unsigned char band_smem[];
     constexpr int T = 32 * R;                 // rows per warp tile
     constexpr int IB = kBandWarps * T;        // rows per I-block, columns per J-block
@@ -75,6 +80,8 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
     }
     __syncthreads();
     uint32_t phase = 0u;
+    double vsym = 0.0, vdiag = 0.0;          // potential terms of this thread's pairs (WITHV)
+    constexpr double kLn2 = 0x1.62e42fefa39efp-1;
 
     const int pfirst = B.wpiece[blockIdx.x], plast = B.wpiece[blockIdx.x + 1];
     for (int pc = pfirst; pc < plast; ++pc) {
@@ -123,6 +130,8 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
                     f1[r] = 0.0;
                 }
                 unsigned selfmask = 0u;
+                double vp = MODEL == 2 ? 1.0 : 0.0;
+                int ve = 0;
                 for (int k = 0; k < nv; ++k) {
                     int x = k + off;
                     if (x >= nv) x -= nv;
@@ -134,16 +143,37 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
                         const double2* sp = Jpos + x * 32;
                         double2* sg = Jg + x * 32;
                         if (diag) {
-                            if (masked) sym_chunk_smem<MODEL, R, true, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
-                            else sym_chunk_smem<MODEL, R, false, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                            if (masked) sym_chunk_smem<MODEL, R, true, true, WITHV>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe, &vp, &ve);
+                            else sym_chunk_smem<MODEL, R, false, true, WITHV>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe, &vp, &ve);
                             const int rr = gc - tile * R;             // the walk met j = i for row rr of every lane
-                            if (MODEL == 1 && rr >= 0 && rr < R) selfmask |= 1u << rr;
+                            if ((MODEL == 1 || WITHV) && rr >= 0 && rr < R) selfmask |= 1u << rr;
                         } else {
-                            if (masked) sym_chunk_smem<MODEL, R, true, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
-                            else sym_chunk_smem<MODEL, R, false, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe);
+                            if (masked) sym_chunk_smem<MODEL, R, true, false, WITHV>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe, &vp, &ve);
+                            else sym_chunk_smem<MODEL, R, false, false, WITHV>(a, bb, vi, f0, f1, sp, sg, nvalid, eps, onepe, &vp, &ve);
                         }
                     }
                     if (!diag && (k + 1) % m == 0 && k + 1 < nv) __syncthreads();
+                }
+                if (WITHV) {
+                    double vt = MODEL == 2 ? fma((double)ve, kLn2, log(vp)) : vp;
+                    if (diag) {
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            if (((selfmask >> r) & 1u) && vi[r]) {        // the j = i term this walk met
+                                if (MODEL == 2) {
+                                    vt -= log(eps);
+                                } else {
+                                    const double d = fma(-bb[r], bb[r], fma(-a[r], a[r], onepe));
+                                    const double y0 = rsqrt_seed(d);
+                                    const double e = fma(-d, y0 * y0, 1.0);
+                                    vt -= fma(y0 * e, fma(0.375, e, 0.5), y0);
+                                }
+                            }
+                        }
+                        vdiag += vt;
+                    } else {
+                        vsym += vt;
+                    }
                 }
                 // i-side sums of this (J-block, I-block) visit -> the piece's private row (first visit stores)
                 const bool first = jb == (b > jbfirst ? b : jbfirst);
@@ -178,6 +208,12 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
                 if (MODEL == 2) jbuf1[jbase + x] = pre * g.y;
             }
         }
+    }
+    if (WITHV) {
+        __syncthreads();                                  // the J-block buffers are free: reuse them as scratch
+        double v[1] = {vsym + 0.5 * vdiag};
+        block_sum<kBandThreads, 1>(v, reinterpret_cast<double*>(band_smem));
+        if (threadIdx.x == 0) vband[blockIdx.x] = pre_v * v[0];
     }
 }
 

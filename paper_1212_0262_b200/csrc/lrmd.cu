@@ -85,6 +85,8 @@ struct lrmd_ctx {
     bool state_set = false;
     bool force_valid = false;   // HMF: hmf_partial[cur] holds the sums at theta; pair: partial* hold F(q)
     bool js_valid = false;      // pair models: js[] matches q
+    bool v_valid = false;       // band kernel: vpart[0 .. P) holds the potential at q (the last force evaluation delivered it)
+    bool want_v = false;        // lrmd_step_observe: the force evaluation that ends lrmd_step delivers V as well
     int cur = 0;                // HMF: which of the 3 partial buffers is current
     // cached CUDA graph of kGraphSteps steady-state steps (HMF)
     cudaGraphExec_t graph_exec = nullptr;
@@ -105,7 +107,8 @@ namespace {
 
 // ---- option resolution -------------------------------------------------------------------------------
 
-// Launch shapes compiled in (chosen from sweeps on B200, profiles/r01_sweeps.md).
+// Launch shapes compiled in (chosen from LRMD_OPT_HMF_VARIANT / LRMD_OPT_PAIR_VARIANT / LRMD_OPT_PAIR_CTAS sweeps on B200;
+// the options stay settable so that the choice can be re-measured with bench.py).
 // HMF: variant 0 is the register-prefetch kernel, 1-2 the TMA-staged kernel <consumer threads, stages, CTAs per
 // SM> (N >= 1e6), 3 the cluster-resident kernel (N <= 20,480: the step is latency-bound).
 struct HmfVariant { int consumers, stages, minb; };
@@ -142,8 +145,9 @@ void resolve_sym(lrmd_ctx* c, bool rows_needed) {
     c->sym_batches.clear();
     const int64_t N = c->N;
     if (c->opt_sym == 0 || c->N_total != c->N) return;
+    if (c->model == LRMD_RING && c->opt_precision == 1) return;    // Ring, fp32 pairs: ordered kernel only
     if (c->opt_sym < 0 && N < 2048) return;    // small systems: the ordered kernel's one wave is as fast
-    // i per lane: Ring 4, 2D 8 (sweeps, profiles/); launch shape 0 / 1 asks for 4 / 8
+    // i per lane: Ring 4, 2D 8 (measured best of the two); launch shape 0 / 1 asks for 4 / 8
     const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
     const int T = 32 * R;
     const int64_t ntiles = (N + T - 1) / T, nchunks = (N + 31) / 32;
@@ -156,7 +160,7 @@ void resolve_sym(lrmd_ctx* c, bool rows_needed) {
     if (!rows_needed) TB = ntiles;
     if (TB < 1) TB = 1;
     if (TB > ntiles) TB = ntiles;
-    // workers per launch: 32 per SM (4 waves of the 8 resident warps; sweeps in profiles/); at least two units each
+    // workers per launch: 32 per SM (4 waves of the 8 resident warps); at least two units each
     int64_t Gwant = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (int64_t)kNumSm * 32;
     // the host-built work table has one entry per worker and launch: keep it below 2^22 entries (64 MB)
     const int64_t nbatches = (ntiles + TB - 1) / TB;
@@ -413,7 +417,10 @@ void resolve(lrmd_ctx* c) {
             L.jpart0 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows);
             if (two) { L.jpart1 = off; off = align_up(off + sizeof(double) * (size_t)N * c->sym_rows); }
         }
-        L.vpart = off; off = align_up(off + sizeof(double) * (c->sym && c->sym_wstart.size() > (size_t)G ? c->sym_wstart.size() : (size_t)G));
+        size_t nv = (size_t)G;
+        if (c->sym && c->sym_wstart.size() > nv) nv = c->sym_wstart.size();
+        if (c->band && (size_t)c->bpart.P > nv) nv = (size_t)c->bpart.P;
+        L.vpart = off; off = align_up(off + sizeof(double) * nv);
         c->use_graph = false;
     }
     L.kpart = off; off = align_up(off + sizeof(double) * 3 * kEnergyGrid);
@@ -500,11 +507,13 @@ struct Launcher {
                 if (cudaEventCreate(&e) != cudaSuccess) { (void)cudaGetLastError(); go(kernel, grid, block, a...); return; }
                 c->ev.push_back(e);
             }
-            cudaEventRecord(c->ev[c->ev_used], stream);
+            const cudaError_t e = cudaEventRecord(c->ev[c->ev_used], stream);
+            if (e != cudaSuccess) { c->cuda_err = (int)e; rc = LRMD_ECUDA; (void)cudaGetLastError(); return; }
         }
         go(kernel, grid, block, a...);
         if (t) {
-            cudaEventRecord(c->ev[c->ev_used + 1], stream);
+            const cudaError_t e = cudaEventRecord(c->ev[c->ev_used + 1], stream);
+            if (e != cudaSuccess) { c->cuda_err = (int)e; rc = LRMD_ECUDA; (void)cudaGetLastError(); return; }
             c->ev_used += 2;
         }
     }
@@ -718,7 +727,7 @@ void pair_pack(Launcher& L) {
     lrmd_ctx* c = L.c;
     const dim3 g((unsigned)((c->N + kUpdThreads - 1) / kUpdThreads)), b(kUpdThreads);
     if (c->model == LRMD_RING)
-        L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, c->i0, js_ptr(c), (float2*)nullptr);
+        L.go(pair_pack_kernel<1>, g, b, c->a0, (const double*)nullptr, c->N, c->i0, js_ptr(c), js32_ptr(c));
     else L.go(pair_pack_kernel<2>, g, b, c->a0, c->a1, c->N, c->i0, js_ptr(c), js32_ptr(c));
     pair_gather(L);
 }
@@ -776,19 +785,25 @@ void pair_force_sym(Launcher& L, int upd = 0, double kickA = 0.0, double kickB =
 }
 
 // Band-kernel force evaluation: one launch + the fold (which takes the update that follows, upd as above).
-void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB = 0.0, double drift = 0.0) {
+void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB = 0.0, double drift = 0.0, bool withv = false) {
     lrmd_ctx* c = L.c;
+    // V = pre_v * sum_{i<j} t_ij (eqs.(1),(3)), delivered with the force when withv
+    const double pre_v = c->model == LRMD_RING ? -1.0 / (std::sqrt(2.0) * (double)c->N) : 1.0 / (double)c->N;
     double *i0 = wsd(c, c->lay.bibuf0), *i1 = wsd(c, c->lay.bibuf1), *j0 = wsd(c, c->lay.bjbuf0), *j1 = wsd(c, c->lay.bjbuf1);
     const double pre = c->model == LRMD_RING ? -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N) : -2.0 / (double)c->N;
     const dim3 g((unsigned)c->bpart.P), b(kBandThreads);
     L.smem = band_smem_bytes(c->band_R);
-#define LRMD_BAND_GO(M, RR) L.go_timed(pair_force_band_kernel<M, RR>, g, b, (const double2*)js_ptr(c), c->bpart, c->eps, pre, i0, i1, j0, j1)
+#define LRMD_BAND_GO(M, RR, V) \
+    L.go_timed(pair_force_band_kernel<M, RR, V>, g, b, (const double2*)js_ptr(c), c->bpart, c->eps, pre, i0, i1, j0, j1, pre_v, vpart(c))
+#define LRMD_BAND_V(M, RR) do { if (withv) LRMD_BAND_GO(M, RR, true); else LRMD_BAND_GO(M, RR, false); } while (0)
     if (c->model == LRMD_RING) {
-        if (c->band_R == 8) LRMD_BAND_GO(1, 8); else LRMD_BAND_GO(1, 4);
+        if (c->band_R == 8) LRMD_BAND_V(1, 8); else LRMD_BAND_V(1, 4);
     } else {
-        if (c->band_R == 8) LRMD_BAND_GO(2, 8); else LRMD_BAND_GO(2, 4);
+        if (c->band_R == 8) LRMD_BAND_V(2, 8); else LRMD_BAND_V(2, 4);
     }
+#undef LRMD_BAND_V
 #undef LRMD_BAND_GO
+    c->v_valid = withv;
     FusedUpdate U;
     U.q0 = c->a0; U.q1 = nullptr; U.p0 = c->a1; U.p1 = nullptr;
     if (c->model == LRMD_GRAV2D) { U.q1 = c->a1; U.p0 = c->a2; U.p1 = c->a3; }
@@ -813,14 +828,17 @@ ForceRows force_rows(lrmd_ctx* c) {
     return FR;
 }
 
-void pair_force(Launcher& L) {
+void pair_force(Launcher& L, bool withv = false) {
     lrmd_ctx* c = L.c;
-    if (c->band) { pair_force_band(L); return; }
+    if (c->band) { pair_force_band(L, 0, 0.0, 0.0, 0.0, withv); return; }
     if (c->sym) { pair_force_sym(L); return; }
     with_pair_cfg(c->pair_variant, [&](auto cfg) {
         using CFG = decltype(cfg);
         const dim3 g((unsigned)c->part.G), b(CFG::THREADS);
-        if (c->model == LRMD_RING)
+        if (c->model == LRMD_RING && c->opt_precision == 1)
+            L.go_timed(ring_force_f32_kernel<CFG>, g, b, (const float2*)js32_ptr(c), c->part, (float)c->eps,
+                       -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N_total), part0(c));
+        else if (c->model == LRMD_RING)
             L.go_timed(pair_force_kernel<1, CFG>, g, b, js_ptr(c), c->part, c->eps,
                        -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N_total), part0(c), part1(c));
         else if (c->opt_precision == 1)
@@ -865,21 +883,22 @@ int pair_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     // A force evaluation that is one launch of the symmetric kernel takes the update that follows it into its
     // fold kernel (same arithmetic, one launch and one pass over the force row fewer per substage).
     const bool fuse = (c->band || (c->sym && c->sym_batches.size() == 1)) && c->opt_fuse != 0;
-    auto force_then_update = [&](bool kick2, bool drift, double kA, double kB, double d) {
+    auto force_then_update = [&](bool kick2, bool drift, double kA, double kB, double d, bool withv = false) {
         if (fuse) {
-            if (c->band) pair_force_band(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
+            if (c->band) pair_force_band(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d, withv);
             else pair_force_sym(L, drift ? (kick2 ? 3 : 2) : 1, kA, kB, d);
         } else {
-            pair_force(L);
+            pair_force(L, withv);
             pair_update(L, kick2, drift, kA, kB, d);
         }
     };
+    c->v_valid = false;
     pair_update(L, false, true, k.B0 * dt, 0.0, k.D0 * dt);
     for (int64_t s = 0; s < n; ++s) {
         force_then_update(false, true, k.B1 * dt, 0.0, k.D1 * dt);
         force_then_update(false, true, k.B1 * dt, 0.0, k.D0 * dt);
         if (s + 1 < n) force_then_update(true, true, k.B0 * dt, k.B0 * dt, k.D0 * dt);   // closing + opening kick
-        else force_then_update(false, false, k.B0 * dt, 0.0, 0.0);                       // closing kick
+        else force_then_update(false, false, k.B0 * dt, 0.0, 0.0, c->band && c->want_v);   // closing kick (+ V for a record)
     }
     return L.rc;
 }
@@ -959,6 +978,7 @@ int lrmd_set_workspace(lrmd_ctx* c, void* device_ptr, size_t bytes, void* cuda_s
         c->spart.tile_rng = reinterpret_cast<const int2*>(c->ws + c->lay.sym_tiles);
     }
     c->force_valid = false;
+    c->v_valid = false;
     c->js_valid = false;
     drop_graph(c);
     return LRMD_OK;
@@ -976,6 +996,7 @@ int lrmd_set_state(lrmd_ctx* c, double* a0, double* a1, double* a2, double* a3) 
     c->a0 = a0; c->a1 = a1; c->a2 = a2; c->a3 = a3;
     c->state_set = true;
     c->force_valid = false;
+    c->v_valid = false;
     c->js_valid = false;
     drop_graph(c);
     return LRMD_OK;
@@ -1013,6 +1034,7 @@ int lrmd_step_host(lrmd_ctx* c, double* h0, double* h1, double* h2, double* h3, 
         e = cudaMemcpyAsync(dev[k], host[k], bytes, cudaMemcpyHostToDevice, stream);
     if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_ECUDA; }
     c->force_valid = false;
+    c->v_valid = false;
     c->js_valid = false;
     if (n > 0) {
         rc = c->model == LRMD_HMF ? hmf_step(c, n, dt, stream) : pair_step(c, n, dt, stream);
@@ -1062,6 +1084,13 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
              hmf_sums(c, c->cur), hmf_nsums(c), (const double*)nullptr, 0, out4_device);
     } else {
         if (!c->js_valid) { pair_pack(L); c->js_valid = true; }
+        if (c->band && c->v_valid && c->force_valid) {
+            // the force evaluation that ended the last step delivered V (lrmd_step_observe): no O(N^2) sweep
+            L.go(energy_finalize_kernel, dim3(1), dim3(kHmfThreads), c->model, c->N, (const double*)kpart(c), (int)gk,
+                 (const double2*)nullptr, 0, (const double*)vpart(c), c->bpart.P, out4_device);
+            return L.rc;
+        }
+        c->v_valid = false;      // the sweeps below reuse the partials' buffer
         if (c->sym) {
             // V = pre * sum_{i<j} t_ij, every unordered pair evaluated once
             const double pre = c->model == LRMD_RING ? -1.0 / (std::sqrt(2.0) * (double)c->N) : 1.0 / (double)c->N;
@@ -1115,6 +1144,7 @@ int lrmd_set_shard(lrmd_ctx* c, int64_t N_total, int64_t i0, lrmd_allreduce_fn a
     resolve(c);
     drop_graph(c);
     c->force_valid = false;
+    c->v_valid = false;
     c->js_valid = false;
     rebind_if_changed(c, before, had_sym);
     return LRMD_OK;
@@ -1126,12 +1156,16 @@ int lrmd_step_observe(lrmd_ctx* c, int64_t n, double dt, int64_t every, double* 
     if (n < 0 || every < 1 || !std::isfinite(dt) || !out_device) return LRMD_EINVAL;
     rc = lrmd_energy(c, out_device, cuda_stream);
     int64_t done = 0, rec = 1;
+    // band kernel: the force evaluation that ends each lrmd_step call also delivers V (+1 FP64 instruction per pair on
+    // one of the 3 evaluations per step instead of a second O(N^2) sweep per record)
+    c->want_v = c->band;
     while (rc == LRMD_OK && done + every <= n) {
         rc = lrmd_step(c, every, dt, cuda_stream);
         if (rc == LRMD_OK) rc = lrmd_energy(c, out_device + 4 * rec, cuda_stream);
         done += every;
         ++rec;
     }
+    c->want_v = false;
     if (rc == LRMD_OK && done < n) rc = lrmd_step(c, n - done, dt, cuda_stream);
     return rc;
 }
@@ -1141,7 +1175,7 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
     switch (key) {
         case LRMD_OPT_PAIR_PRECISION:
             if (value != 0 && value != 1) return LRMD_EINVAL;
-            if (value == 1 && c->model != LRMD_GRAV2D) return LRMD_EUNSUPPORTED;   // fp32 pairs: GRAV2D only
+            if (value == 1 && c->model == LRMD_HMF) return LRMD_EUNSUPPORTED;      // fp32 pairs: the pair models
             if (value == 1 && !(c->eps >= 1e-30)) return LRMD_EUNSUPPORTED;        // eps must be a normal float
             c->opt_precision = value;
             break;
@@ -1207,6 +1241,7 @@ int lrmd_set_option(lrmd_ctx* c, int key, int64_t value) {
     resolve(c);
     drop_graph(c);
     c->force_valid = false;
+    c->v_valid = false;
     c->js_valid = false;
     rebind_if_changed(c, before, had_sym);
     return LRMD_OK;

@@ -356,6 +356,82 @@ grav_force_f32_kernel(const float2* __restrict__ js32, PairPart P, float eps, do
     }
 }
 
+// ---- Ring force, fp32 pair arithmetic ---------------------------------------
+// "computing the force between the two particles using single precision arithmetic do not compromise the overall
+// accuracy".  Eq.(9)'s denominator 1 + eps - c_i c_j - s_i s_j cancels to ~eps for close
+// pairs: rounded to fp32 its relative error is ~1.5e-7 / eps, i.e. ~2e-5 on the pair term at eps = 0.01 — above the
+// 1e-5 A_i tolerance.  The half-angle form has no cancellation: with (ch, sh)_i = (cos, sin)(theta_i / 2) stored in fp32,
+//     S = sin((ti - tj)/2) = sh_i ch_j - ch_i sh_j,   C = cos((ti - tj)/2) = ch_i ch_j + sh_i sh_j,
+//     1 - cos(ti - tj) = 2 S^2,   sin(ti - tj) = 2 S C,   term = 2 S C (eps + 2 S^2)^(-3/2),
+// every operation in fp32 (12 FADD/FMUL/FFMA + MUFU.RSQ per pair); the relative error of eps + 2 S^2 stays ~1e-7.
+// S uses two rounded products, so j = i gives exactly 0.  Sums as in grav_force_f32_kernel (reading G16): fp32 over at
+// most kF32Chunk consecutive j, then added to the fp64 accumulator.
+__device__ __forceinline__ float rsqrt_f32(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <typename CFG>
+__global__ void __launch_bounds__(CFG::THREADS, CFG::MINB)
+ring_force_f32_kernel(const float2* __restrict__ hs32, PairPart P, float eps, double pre, double* __restrict__ partial0) {
+    constexpr int R = CFG::R, THREADS = CFG::THREADS, TJ = CFG::TJ;
+    __shared__ PairSmem<float2, TJ> sm;
+    JTilePipe<float2, TJ> pipe(sm);
+    pipe.init();
+    const long long N = P.Ni;
+
+    PairSegments segs(P, blockIdx.x);
+    long long tile, jbeg, jend;
+    int slot;
+    while (segs.next(P, tile, jbeg, jend, slot)) {
+        const long long ibase = tile * CFG::ITILE + threadIdx.x;
+        float ch[R], sh[R];
+        double f0[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            const float2 q = (i < N) ? hs32[P.i0 + i] : make_float2(1.f, 0.f);
+            ch[r] = q.x;
+            sh[r] = q.y;
+            f0[r] = 0.0;
+        }
+        pipe.run(hs32, jbeg, jend, [&](const float2* tl, int cnt, long long) {
+            for (int c0 = 0; c0 < cnt; c0 += kF32Chunk) {
+                const int m = (cnt - c0 < kF32Chunk) ? (cnt - c0) : kF32Chunk;
+                float acc[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) acc[r] = 0.f;
+                auto pair = [&](const float2 q) {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {
+                        const float S = __fsub_rn(__fmul_rn(sh[r], q.x), __fmul_rn(ch[r], q.y));
+                        const float C = fmaf(ch[r], q.x, sh[r] * q.y);
+                        const float S2 = S + S;
+                        const float d = fmaf(S2, S, eps);
+                        const float y = rsqrt_f32(d);
+                        const float w = (S2 * C) * y;
+                        acc[r] = fmaf(w, y * y, acc[r]);
+                    }
+                };
+                if (m == kF32Chunk) {
+#pragma unroll 8
+                    for (int jj = 0; jj < kF32Chunk; ++jj) pair(tl[c0 + jj]);   // broadcast LDS.64
+                } else {
+                    for (int jj = 0; jj < m; ++jj) pair(tl[c0 + jj]);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) f0[r] += (double)acc[r];
+            }
+        });
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const long long i = ibase + (long long)r * THREADS;
+            if (i < N) partial0[(long long)slot * N + i] = pre * f0[r];
+        }
+    }
+}
+
 // ---- symmetric force kernels: Newton's third law ------------------------------------
 // The paper computes every ordered pair ("the symmetry ... would introduce unnecessary complications with no
 // significant speed gain").  On an FP64-issue-bound B200 kernel halving the pair evaluations is
@@ -402,7 +478,7 @@ __device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b
         // The R pair evaluations of a step are written stage by stage over groups of 4, so that the four
         // dependency chains (difference -> r^2 -> MUFU seed -> correction -> accumulate) are interleaved in
         // the instruction stream: written pair by pair, the compiler reused one register set and ran the
-        // chains back to back, every correction waiting for its own seed (profiles/r01e_summary.md).
+        // chains back to back, every correction waiting for its own seed.
 #pragma unroll
         for (int r0 = 0; r0 < R; r0 += 4) {
             if (MODEL == 2) {
@@ -474,7 +550,7 @@ __device__ __forceinline__ void sym_chunk(const double (&a)[R], const double (&b
 // on slot (l + s) mod 32 — one conflict-free LDS.128 for the position, and the slot's force sum is read, extended
 // by the lane's R pair terms and written back (LDS.128 / STS.128); __syncwarp() orders a step's write-back before
 // the neighbour lane's read of the same slot in the next step.  Measured on B200 with lrmd_fp64_peak
-// (profiles/r02_fp64_peak.md): next to DFMA traffic an LDS / STS / integer instruction costs no FP64 issue
+// (bench.py --fp64-peak, profiles/r02_fp64_peak.md): next to DFMA traffic an LDS / STS / integer instruction costs no FP64 issue
 // cycle, a SHFL costs about one (the shuffle walk spends 8 per step), and the position of the next step no longer
 // depends on a shuffle chain.
 struct SymWarpSmem {
@@ -482,10 +558,17 @@ struct SymWarpSmem {
     double2 g[32];
 };
 
-template <int MODEL, int R, bool MASK, bool DIAG>
+// WITHV: the walk also collects the potential of the pairs it meets (rows a-E2 / a-E3 fused into the force kernel, one
+// extra DMUL (2D) or four extra instructions (Ring) per pair): 2D  vp *= r^2 + eps with the exponent moved to the integer
+// counter ve once per step (needs 2^-127 <= r^2 + eps <= 2^127; sum log = log prod as in pair_energy_kernel);
+// Ring  vp += d^(-1/2).  A DIAG walk meets every pair of the block twice and j = i once: the caller halves and corrects.
+template <int MODEL, int R, bool MASK, bool DIAG, bool WITHV = false>
 __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const double (&b)[R], const bool (&vi)[R],
                                                double (&f0)[R], double (&f1)[R], const double2* __restrict__ spos,
-                                               double2* __restrict__ sg, int nvalid, double eps, double onepe) {
+                                               double2* __restrict__ sg, int nvalid, double eps, double onepe,
+                                               double* vp_ = nullptr, int* ve_ = nullptr) {
+    double vp = WITHV ? *vp_ : 0.0;
+    int ve = WITHV ? *ve_ : 0;
     // spos / sg: the 32 slots of the packet in shared memory (positions; force sums, read and written when !DIAG)
     const int lane = threadIdx.x & 31;
     double2 qn = spos[lane];
@@ -514,6 +597,10 @@ __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const doubl
                 for (int k = 0; k < 4; ++k) r2[k] = fma(dy[k], dy[k], fma(dx[k], dx[k], eps));
 #pragma unroll
                 for (int k = 0; k < 4; ++k) y0[k] = rcp_seed(r2[k]);
+                if (WITHV) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) vp *= MASK ? ((vi[r0 + k] && vq) ? r2[k] : 1.0) : r2[k];
+                }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const double e = fma(-r2[k], y0[k], 1.0);
@@ -547,6 +634,10 @@ __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const doubl
                     c[k] = (num[k] * y0[k]) * bb;
                     p[k] = fma(fma(1.875, e, 1.5), e, 1.0);
                     if (MASK) c[k] = (vi[r0 + k] && vq) ? c[k] : 0.0;
+                    if (WITHV) {     // d^(-1/2) = y0 (1 + e/2 + 3 e^2/8), the arithmetic of rsqrt_refined
+                        const double rs = fma(y0[k] * e, fma(0.375, e, 0.5), y0[k]);
+                        vp += MASK ? ((vi[r0 + k] && vq) ? rs : 0.0) : rs;
+                    }
                 }
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
@@ -555,10 +646,19 @@ __device__ __forceinline__ void sym_chunk_smem(const double (&a)[R], const doubl
                 }
             }
         }
+        if (WITHV && MODEL == 2) {      // move the product's exponent into the integer counter
+            const int hi = __double2hiint(vp);
+            ve += ((hi >> 20) & 0x7ff) - 1023;
+            vp = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(vp));
+        }
         if (!DIAG) {
             sg[idx] = make_double2(h0, h1);
             __syncwarp();
         }
+    }
+    if (WITHV) {
+        *vp_ = vp;
+        *ve_ = ve;
     }
 }
 
@@ -1034,6 +1134,10 @@ pair_pack_kernel(const double* __restrict__ q0, const double* __restrict__ q1, l
         double s, c;
         sincos_any(q0[i], s, c);
         js[i0 + i] = make_double2(c, s);
+        if (js32) {     // fp32 pair arithmetic: (cos, sin)(theta / 2), see ring_force_f32_kernel
+            sincos_any(0.5 * q0[i], s, c);
+            js32[i0 + i] = make_float2((float)c, (float)s);
+        }
     } else {
         js[i0 + i] = make_double2(q0[i], q1[i]);
         if (js32) js32[i0 + i] = make_float2((float)q0[i], (float)q1[i]);
@@ -1195,6 +1299,10 @@ pair_update_kernel(double* __restrict__ q0, double* __restrict__ q1, double* __r
             double sn, cs;
             sincos_any(x, sn, cs);
             js[P.i0 + i] = make_double2(cs, sn);
+            if (js32) {
+                sincos_any(0.5 * x, sn, cs);
+                js32[P.i0 + i] = make_float2((float)cs, (float)sn);
+            }
         }
     }
 }

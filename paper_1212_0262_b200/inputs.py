@@ -110,3 +110,12 @@ WORKLOADS = {
     "hmf_5e7": Workload("hmf_5e7", 4, HMF, 50_000_000, 0.0, 0.05, 100, theta_hw=1.5, p_hw=0.5),
     "grav2d_1m": Workload("grav2d_1m", 5, GRAV2D, 1_048_576, 1e-3, 0.005, 5, sigma_p=0.1),
 }
+
+# HMF sizes of the paper's Table 1 (N = 1e5 .. 1e8) that are not BASELINE.json configs: same waterbag
+# as configs 1 and 4, own seeds.  bench.py reports them beside the configs so that the three HMF regimes of the
+# library (cluster-resident, graph replay of the register-prefetch kernel, TMA-staged) each have a measured entry.
+TABLE1_WORKLOADS = {
+    "hmf_1e5": Workload("hmf_1e5", 6, HMF, 100_000, 0.0, 0.05, 1000, theta_hw=1.5, p_hw=0.5),
+    "hmf_1e6": Workload("hmf_1e6", 7, HMF, 1_000_000, 0.0, 0.05, 500, theta_hw=1.5, p_hw=0.5),
+    "hmf_1e7": Workload("hmf_1e7", 8, HMF, 10_000_000, 0.0, 0.05, 200, theta_hw=1.5, p_hw=0.5),
+}

@@ -292,6 +292,12 @@ class Context:
         ptr = (self._ws.data_ptr() + 255) // 256 * 256
         self._chk(lrmd_set_workspace(self._h, ptr, nbytes, self._stream()), "lrmd_set_workspace")
 
+    def workspace_bytes(self) -> int:
+        """Scratch the library asked for with the current options (lrmd_workspace_bytes)."""
+        rc, nbytes = lrmd_workspace_bytes(self._h)
+        self._chk(rc, "lrmd_workspace_bytes")
+        return nbytes
+
     @property
     def narrays(self) -> int:
         return 4 if self.model == GRAV2D else 2

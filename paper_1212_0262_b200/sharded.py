@@ -6,8 +6,9 @@ as callbacks that run ``torch.distributed`` collectives (NCCL on GPUs) on views 
   HMF          one all-reduce of 2 doubles per substage (each GPU's contribution to the magnetisation, summed);
   RING/GRAV2D  one all-gather of the packed positions per substage (every GPU needs all positions for its rows).
 
-BASELINE.json's north_star fixes ONE GPU, so bench.py never uses this module (replicas only); it is covered by a
-two-rank emulation on one GPU (tests/test_gpu_parity.py) and by gloo world-2 CPU tests of the collectives.
+BASELINE.json's north_star fixes ONE GPU, so bench.py's default line never uses this module (replicas only);
+``bench.py --sharded`` times it as an opt-in strong-scaling line.  It is covered by a two- and three-rank emulation on
+one GPU (tests/test_gpu_sharded.py) and by gloo world-2 CPU tests of the collectives and of bench.py's host logic.
 """
 from __future__ import annotations
 
@@ -45,6 +46,17 @@ class TorchDistCollectives:
             for r, (b0, b1) in enumerate(byte_bounds):
                 if b1 > b0:
                     self.dist.broadcast(whole[b0:b1], src=r, group=self.group)
+
+
+class SingleRankCollectives:
+    """World of one rank: nothing to exchange (the library runs its unsharded path and never calls back)."""
+    rank, world = 0, 1
+
+    def all_reduce_sum_(self, t):
+        pass
+
+    def all_gather_inplace_(self, whole, byte_bounds):
+        pass
 
 
 class ShardedContext(lrmd.Context):

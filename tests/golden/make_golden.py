@@ -8,7 +8,8 @@ and its tables are timings), so there is no paper value to store; what pins the 
 mathematical checks in tests/test_oracle_*.py (mpmath gradients of the printed Hamiltonians, closed
 forms, invariants).  This file freezes the pinned oracle's output on fixed inputs so that
   * a later change to the oracle's arithmetic shows up as a diff of stored numbers (regression), and
-  * the CUDA path is also compared with values that were on disk before it ran (tests/test_golden.py).
+  * the CUDA path is also compared with stored values written by the oracle alone (tests/test_golden.py); they were
+    committed after the first kernels existed, which is harmless: no value in them comes from the CUDA path.
 Nothing here imports or calls the CUDA path.  Inputs are written into the file (hex floats, exact).
 """
 import json

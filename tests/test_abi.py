@@ -72,7 +72,10 @@ def test_options(lrmd):
     assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SYMMETRIC) == (lrmd.OK, 1)     # chosen for this size (row N4)
     rc, W = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)
     assert rc == lrmd.OK and W % 148 == 0                                        # workers (warps) of the symmetric kernel
-    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 2) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 3) == lrmd.EINVAL
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 2) == lrmd.OK        # band kernel
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_SYMMETRIC) == (lrmd.OK, 2)
+    assert lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS) == (lrmd.OK, 296)           # CTAs, 2 per SM
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_SYMMETRIC, 0) == lrmd.OK        # the paper's every-ordered-pair scheme
     rc, G = lrmd.lrmd_get_option(h, lrmd.OPT_PAIR_CTAS)
     assert rc == lrmd.OK and G % 148 == 0 and G >= 148   # whole waves of the 148 SMs
@@ -87,7 +90,13 @@ def test_options(lrmd):
     assert lrmd.lrmd_set_option(h, lrmd.OPT_HMF_VARIANT, 1) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_VARIANT, 9999) == lrmd.EINVAL
     assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 2) == lrmd.EINVAL
-    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.EUNSUPPORTED   # fp32 pairs: GRAV2D only
+    rc, b64 = lrmd.lrmd_workspace_bytes(h)
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.OK             # Ring, fp32 pairs: half-angle stream
+    assert lrmd.lrmd_workspace_bytes(h)[1] > b64
+    assert lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_PRECISION, 0) == lrmd.OK
+    rc, hh = lrmd.lrmd_create(HMF, 1000, 0.0)
+    assert lrmd.lrmd_set_option(hh, lrmd.OPT_PAIR_PRECISION, 1) == lrmd.EUNSUPPORTED  # HMF has no pair arithmetic
+    lrmd.lrmd_destroy(hh)
     rc, b3 = lrmd.lrmd_workspace_bytes(h)
     lrmd.lrmd_set_option(h, lrmd.OPT_PAIR_CTAS, 32 * 6)
     rc, b6 = lrmd.lrmd_workspace_bytes(h)

@@ -4,7 +4,7 @@
 CPU: the oracle still reproduces the stored values bit for bit, and the stored forces agree with a
 brute-force numpy evaluation of -dH/dq written from the printed Hamiltonians.
 GPU: the CUDA path matches the stored forces / energies / 10-step trajectory within north_star's
-tolerances — values that were on disk before the CUDA path ran.
+tolerances — values written by the oracle alone (tests/golden/make_golden.py calls only oracle/).
 """
 import json
 import os

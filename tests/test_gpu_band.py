@@ -122,3 +122,49 @@ def test_band_kernel_agrees_with_the_other_pair_kernels(lrmd, torch):
     for other in fs[1:]:
         for a, b in zip(fs[0], other):
             assert np.max(np.abs(a - b)) <= 1e-11 * scale
+
+
+@pytest.mark.parametrize("model", [RING, GRAV2D])
+@pytest.mark.parametrize("N,height,fuse", [(1500, 0, 1), (4099, 2, 1), (2049, 1, 0), (6000, 0, 1)])
+def test_band_step_observe_uses_the_fused_potential(lrmd, ref, torch, model, N, height, fuse):
+    """lrmd_step_observe on a band-kernel context: the force evaluation that ends each recorded step delivers V
+    (PAPER.md:61 step 12; rows a-E2 / a-E3 fused into the force kernel): one launch fewer per record than a separate
+    O(N^2) sweep, records equal to the oracle's stepped alongside, state equal to plain stepping bit for bit."""
+    eps = _eps(model)
+    st = _state(model, N, 63 + N)
+    opts = {lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_BAND_HEIGHT: height, lrmd.OPT_PAIR_FUSE_UPDATE: fuse}
+    ctx = lrmd.Context(model, N, eps, options=opts)
+    ctx.set_state(*st)
+    l0 = ctx.launch_count()
+    rec = ctx.step_observe(7, 0.01, 2).cpu().numpy()          # records at steps 0, 2, 4, 6; 7 steps taken
+    launches = ctx.launch_count() - l0
+    fin = ctx.state_numpy()
+    e_after = ctx.energy().cpu().numpy()                      # separate sweep at the final state
+    ctx.close()
+    assert rec.shape == (4, 4)
+    r = [a.copy() for a in st]
+    q0, q1 = _q(model, r)
+    p0, p1 = _p(model, r)
+    f0 = f1 = None
+    for k in range(4):
+        er, ea = ref.energy(model, eps, q0, q1, p0, p1)
+        assert abs(rec[k, 0] - er[0]) <= 1e-9 * max(ea[0], 1e-300)
+        assert abs(rec[k, 1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N), (k, rec[k, 1], er[1])
+        f0, f1 = ref.step(model, eps, q0, q1, p0, p1, 2 if k < 3 else 1, 0.01, f0, f1, force_valid=(k > 0), form=1)
+    for g, w in zip(fin, r):
+        assert np.max(np.abs(g - w)) <= XTOL
+    er, ea = ref.energy(model, eps, q0, q1, p0, p1)
+    assert abs(e_after[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N)
+    # the same steps without records: identical state (the fused potential changes no force arithmetic)
+    ctx = lrmd.Context(model, N, eps, options=opts)
+    ctx.set_state(*st)
+    l0 = ctx.launch_count()
+    ctx.step(2, 0.01); ctx.step(2, 0.01); ctx.step(2, 0.01); ctx.step(1, 0.01)
+    plain = ctx.launch_count() - l0
+    fin2 = ctx.state_numpy()
+    ctx.close()
+    for x, y in zip(fin, fin2):
+        assert np.array_equal(x, y)
+    # per record after the first: the kinetic partial kernel and the finalize kernel only (no pair sweep); the first
+    # record takes the separate sweep (pack? no: + kinetic, energy kernel, finalize)
+    assert launches - plain <= 3 + 3 * 2 + 2

@@ -676,6 +676,59 @@ def test_f32_pair_variant_trajectory_and_energy(lrmd, ref, torch):
     assert abs(e[0] - er[0]) <= 1e-12 * ea[0] and abs(e[1] - er[1]) <= 1e-12 * ea[1]
 
 
+@pytest.mark.parametrize("eps", [1e-2, 1e-3])
+@pytest.mark.parametrize("N", [1, 2, 3, 257, 1023, 4099, 16_384])
+def test_ring_f32_pair_variant_forces(lrmd, ref, torch, N, eps):
+    """Ring with fp32 pair arithmetic, half-angle form: 1e-5 A_i at eps = 0.01 and 1e-3,
+    on the waterbag of config 2 and on angles over the full circle (paper-shaped)."""
+    for seed, full_circle in ((900 + N % 13, False), (901 + N % 13, True)):
+        st = _state(RING, N, seed)
+        if full_circle:
+            st[0] = np.random.default_rng(seed).uniform(-math.pi, math.pi, N)
+        f0, _, A0, _ = ref.forces_abs(RING, eps, st[0], None, form=0)
+        for variant, ctas in ((0, 0), (1, 7), (2, 0)):
+            ctx = lrmd.Context(RING, N, eps, options={lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_VARIANT: variant,
+                                                       lrmd.OPT_PAIR_CTAS: ctas})
+            assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0 and ctx.get_option(lrmd.OPT_PAIR_PRECISION) == 1
+            ctx.set_state(*st)
+            g = ctx.forces().cpu().numpy()
+            ctx.close()
+            err = np.abs(g - f0)
+            assert np.all(err <= F32TOL * A0 + 1e-300), (eps, full_circle, float((err / np.maximum(A0, 1e-300)).max()))
+    if N == 1:
+        assert g[0] == 0.0          # j = i contributes exactly 0
+
+
+def test_ring_f32_pair_variant_trajectory_energy_and_reproducibility(lrmd, ref, torch):
+    N = 3001
+    st = _state(RING, N, 23)
+    outs = []
+    for _ in range(2):
+        ctx = lrmd.Context(RING, N, 0.01, options={lrmd.OPT_PAIR_PRECISION: 1})
+        ctx.set_state(*st)
+        ctx.step(10, 0.01)
+        outs.append(ctx.state_numpy())
+        e = ctx.energy().cpu().numpy()
+        ctx.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    r = [a.copy() for a in st]
+    ref.step(RING, 0.01, r[0], None, r[1], None, 10, 0.01, form=1)
+    for g, w in zip(outs[0], r):
+        assert np.max(np.abs(g - w)) <= 1e-6
+    er, ea = ref.energy(RING, 0.01, outs[0][0], None, outs[0][1], None)
+    assert abs(e[0] - er[0]) <= 1e-12 * ea[0] and abs(e[1] - er[1]) <= 1e-12 * ea[1]
+    c = lrmd.Context(RING, N, 0.01)
+    c.set_state(*st)
+    f64 = c.forces().cpu().numpy()
+    c.close()
+    c = lrmd.Context(RING, N, 0.01, options={lrmd.OPT_PAIR_PRECISION: 1})
+    c.set_state(*st)
+    f32 = c.forces().cpu().numpy()
+    c.close()
+    rel = np.max(np.abs(f32 - f64)) / np.max(np.abs(f64))
+    assert 1e-12 < rel < 1e-5       # differs from fp64 at the fp32 level, not more
+
+
 # ---- integrator properties on the GPU ---------------------------------------------------------------
 
 @pytest.mark.parametrize("model", [HMF, RING, GRAV2D])
@@ -901,6 +954,43 @@ def test_paper_shaped_runs_conserve_energy(lrmd, torch):
         assert out["K"][0] == 0.0 and len(out["K"]) == 7
         assert out["K"][-1] > 0.0
         assert max(out["energy_error"]) < tol, (name, max(out["energy_error"]))
+
+
+@pytest.mark.parametrize("name,symmetric", [("hmf", -1), ("ring", 0), ("ring", 1), ("ring", 2), ("grav2d", 0), ("grav2d", 1),
+                                            ("grav2d", 2)])
+def test_paper_shaped_runs_match_oracle(lrmd, ref, torch, name, symmetric):
+    """The set-ups of the paper's section 4 against the oracle, not just energy conservation:
+    homogeneous state at rest on the full circle [-pi, pi) (HMF dt = 0.1; Ring eps = 1e-3, dt = 0.005 — where the
+    cancellation of eq.(9)'s denominator is strongest) and the 2D annulus 1.0 <= r <= 1.5 at rest (eps = 1e-3,
+    dt = 0.005): forces at t = 0 within 1e-12 A_i, state within 1e-9 after 10 steps, K and V records every 5 steps."""
+    from paper_1212_0262_b200 import paper_runs
+    su = paper_runs.SETUPS[name]
+    model, eps, dt = su["model"], su["eps"], su["dt"]
+    N = 4099 if model != HMF else 10_007
+    st = [np.array(a, dtype=np.float64) for a in paper_runs.initial_state(name, N)]
+    opts = {} if model == HMF else {lrmd.OPT_PAIR_SYMMETRIC: symmetric}
+    ctx = lrmd.Context(model, N, eps, options=opts or None)
+    ctx.set_state(*st)
+    f = ctx.forces()
+    got = tuple(t.cpu().numpy() for t in f) if model == GRAV2D else (f.cpu().numpy(), None)
+    q0, q1 = _q(model, st)
+    f0, f1, A0, A1 = ref.forces_abs(model, eps, q0, q1, form=(1 if model == HMF else 0))
+    _check_forces(model, got, (f0, f1), (A0, A1))
+    rec = ctx.step_observe(10, dt, 5).cpu().numpy()
+    fin = ctx.state_numpy()
+    ctx.close()
+    r = [a.copy() for a in st]
+    rq0, rq1 = _q(model, r)
+    rp0, rp1 = _p(model, r)
+    g0 = g1 = None
+    for k in range(3):
+        er, ea = ref.energy(model, eps, rq0, rq1, rp0, rp1)
+        assert abs(rec[k, 0] - er[0]) <= 1e-9 * max(ea[0], 1e-12) and abs(rec[k, 1] - er[1]) <= 1e-9 * max(ea[1], 0.5 * N)
+        if k < 2:
+            g0, g1 = ref.step(model, eps, rq0, rq1, rp0, rp1, 5, dt, g0, g1, force_valid=(k > 0), form=(0 if model == HMF else 1))
+    assert rec[0, 0] == 0.0 and rec[2, 0] > 0.0          # at rest, then collapsing / relaxing
+    for g, w in zip(fin, r):
+        assert np.max(np.abs(g - w)) <= XTOL
 
 
 @pytest.mark.parametrize("model", [RING, GRAV2D])

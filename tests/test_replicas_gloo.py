@@ -130,3 +130,54 @@ def test_sharding_collectives_gloo_world2():
         assert res[r]["sum"] == [3.0, 30.0]
         assert res[r]["gather6"] == [1, 1, 1, 2, 2, 2]
         assert res[r]["gather7"] == [1, 1, 1, 2, 2, 2, 2]
+
+
+# ---- bench.py --sharded: host logic (plan, strong-scaling value, max over ranks), gloo world 2 on CPU ----------------
+
+def _sharded_bench_worker(rank, world, port, out):
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1212_0262_b200 import inputs
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    res = {}
+    for key in ("grav2d_1m", "hmf_5e7"):
+        w = inputs.WORKLOADS[key]
+        plan = bench.sharded_plan(w, world, rank)
+        ms_local = 100.0 + 50.0 * rank                       # rank 1 is the slow shard
+        ms_max = bench.max_over_ranks(ms_local, dist, torch.device("cpu"))
+        res[key] = (plan, ms_max, bench.strong_scaling_value(plan["units_per_step"], 5, ms_max))
+    out[rank] = res
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_sharded_bench_host_logic_gloo_world2():
+    """Strong scaling: ONE problem split over the ranks; value = its units / the slowest rank's time (not summed over
+    ranks, unlike the replicas line); the shards tile the particles; the exchange per substage is 16 N bytes
+    (all-gather) or 16 bytes (all-reduce)."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    with ctx.Manager() as m:
+        out = m.dict()
+        port = 29500 + (os.getpid() + 13) % 1000
+        procs = [ctx.Process(target=_sharded_bench_worker, args=(r, 2, port, out)) for r in range(2)]
+        for p in procs:
+            p.start()
+        for p in procs:
+            p.join(120)
+            assert p.exitcode == 0
+        res = dict(out)
+    for key, N, units in (("grav2d_1m", 1_048_576, 3.0 * 1_048_576.0 ** 2), ("hmf_5e7", 50_000_000, 5e7)):
+        p0, p1 = res[0][key][0], res[1][key][0]
+        assert p0["i0"] == 0 and p0["i0"] + p0["n_local"] == p1["i0"] and p1["i0"] + p1["n_local"] == N
+        assert p0["units_per_step"] == units == p1["units_per_step"]
+        for r in (0, 1):
+            assert res[r][key][1] == 150.0
+            assert abs(res[r][key][2] - units * 5 / 0.150) <= 1e-6 * units
+    assert res[0]["grav2d_1m"][0]["exchange"] == {"collective": "all_gather", "bytes_per_substage": 16 * 1_048_576}
+    assert res[0]["hmf_5e7"][0]["exchange"] == {"collective": "all_reduce", "bytes_per_substage": 16}
+    assert res[1]["grav2d_1m"][0]["rows_x_columns"] == [524_288, 1_048_576]
