@@ -280,13 +280,14 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                                 "is context only" % (state_bytes / 1e6))
         elif f32_pairs:
             # fp32 pair arithmetic: one MUFU.RCP per pair on the special-function unit, 16 lanes per SM per clock
-            kernel = "grav_force_sym_f32_kernel" if symk else "grav_force_f32_kernel"
+            kernel = "ring_force_f32_kernel" if w.model == 1 else ("grav_force_sym_f32_kernel" if symk else "grav_force_f32_kernel")
             mufu = float(w.N) * float(w.N) * (0.5 if symk else 1.0)      # executed: one per (un)ordered pair evaluated
             peak = SM_COUNT * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
             achieved = mufu / avg_s / 1e12
             roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "T MUFU.RCP/s",
                     "frac": achieved / peak,
-                    "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: 6 FADD/FFMA per pair",
+                    "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: %d FADD/FMUL/FFMA per pair"
+                                   % (12 if w.model == 1 else 6),
                     "algorithmic_mufu_per_launch": mufu}
             if symk:
                 roof["note"] = ("symmetric fp32 kernel: one MUFU.RCP and 8 FADD/FFMA per UNORDERED pair (N^2/2 evaluations deliver "
@@ -591,7 +592,7 @@ def main():
     ap.add_argument("--only", action="store_true", help="primary workload only (no 'others', no cpu_baseline)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
-    ap.add_argument("--f32-pairs", action="store_true", help="GRAV2D workloads: fp32 pair arithmetic (PAPER.md:110)")
+    ap.add_argument("--f32-pairs", action="store_true", help="pair workloads: fp32 pair arithmetic (PAPER.md:110, 136)")
     ap.add_argument("--fp64-peak", action="store_true", help="run only the FP64 issue-rate microbenchmark and print its table")
     ap.add_argument("--ordered-pairs", action="store_true", help="pair workloads: the paper's scheme, every ordered pair (PAPER.md:108)")
     ap.add_argument("--sharded", action="store_true",
@@ -645,7 +646,7 @@ def main():
             dist_ctx.destroy_process_group()
         return 0
 
-    f32 = bool(args.f32_pairs and w.model == 2)
+    f32 = bool(args.f32_pairs and w.model != 0)
     peak = fp64_peak_summary() if (w.model != 0 and not f32) else None
     # the roofline pass and the end-to-end call repeat the steps: bounded for the seconds-long steps of config 5
     heavy = w.key == "grav2d_1m"
@@ -686,6 +687,8 @@ def main():
         others["grav2d_1m_f32pairs"]["dtype"] = "f32 pair terms, f64 state and accumulation"
         add("grav2d_1m_f32pairs_ordered_pairs", inputs.WORKLOADS["grav2d_1m"], 3, with_e2e=False, f32_pairs=True, ordered_pairs=True,
             roofline_steps=3)
+        add("ring_16k_f32pairs", inputs.WORKLOADS["ring_16k"], DEFAULT_STEPS["ring_16k"], with_e2e=False, f32_pairs=True)
+        others["ring_16k_f32pairs"]["dtype"] = "f32 pair terms (half-angle form), f64 state and accumulation"
         line["others"] = others
         rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
         line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc,

@@ -225,6 +225,7 @@ void resolve_sym(lrmd_ctx* c, bool rows_needed) {
 // 11 (2D) or 12 (Ring) FP64 instructions per pair for every I-block of the band above the block, 9 / 11 for the block
 // itself if it is in the band (DIAG walk: every ordered pair, i-side only).
 constexpr int64_t kBandMinN = 49152;     // default: band kernel from this N on (unsharded fp64 contexts)
+constexpr double kBandL2Bytes = 80.0 * 1048576.0;   // i-side rows all CTAs cycle through: kept within L2
 
 void resolve_band(lrmd_ctx* c) {
     c->band = false;
@@ -240,17 +241,31 @@ void resolve_band(lrmd_ctx* c) {
     const int64_t nIB = (N + IB - 1) / IB, nchunks = (N + 31) / 32;
     if (nIB > (1 << 20)) return;
     const int64_t P = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : 2 * (int64_t)kNumSm;
-    // band height: the i-side rows cost (pieces ~ P + bands) x hb x IB elements, the j-side rows ~ bands x N / 2
+    // band height: the i-side rows cost (pieces ~ P + bands) x hb x IB elements, the j-side rows ~ bands x N / 2.  A CTA
+    // adds to its piece's i-side row once per (J-block, I-block) visit, cycling through hb x IB rows: the height is
+    // capped so that the rows all CTAs cycle through stay in L2 (kBandL2Bytes of the 126 MB), else every visit would
+    // take 64 KB through HBM (8.5 GB per force evaluation at N = 2^20 with the unconstrained height 21; ncu, profiles/).
+    const int comps = c->model == LRMD_GRAV2D ? 2 : 1;
     int64_t hb = 1;
     if (c->opt_band_height > 0) {
         hb = c->opt_band_height < nIB ? c->opt_band_height : nIB;
     } else {
-        double best = -1.0;
-        for (int64_t h = 1; h <= nIB; ++h) {
+        int64_t hmax = (int64_t)(kBandL2Bytes / ((double)P * (double)IB * 8.0 * comps));
+        if (hmax < 1) hmax = 1;
+        auto elements = [&](int64_t h) {
             const double nb = (double)((nIB + h - 1) / h);
-            const double cost = ((double)P + nb) * (double)h * (double)IB + nb * 0.5 * (double)N;
+            return ((double)P + nb) * (double)h * (double)IB + nb * 0.5 * (double)N;
+        };
+        double best = -1.0, best_l2 = -1.0;
+        int64_t h_l2 = 1;
+        for (int64_t h = 1; h <= nIB; ++h) {
+            const double cost = elements(h);
             if (best < 0.0 || cost < best) { best = cost; hb = h; }
+            if (h <= hmax && (best_l2 < 0.0 || cost < best_l2)) { best_l2 = cost; h_l2 = h; }
         }
+        // beyond ~1 GiB of rows the L2-resident height costs more memory than the HBM round trips are worth
+        // (64 KB per 4.2e6 pair evaluations)
+        if (best_l2 * 8.0 * comps <= 1073741824.0) hb = h_l2;
     }
     const int64_t nbands = (nIB + hb - 1) / hb;
     const int64_t wsym = c->model == LRMD_RING ? 12 : 11, wdiag = c->model == LRMD_RING ? 11 : 9;

@@ -365,14 +365,14 @@ def test_config4_hmf_5e7_sampled_and_invariants(lrmd, ref, torch, inputs):
 
 @pytest.mark.parametrize("symmetric", [-1, 0])
 def test_config5_grav2d_1m_sampled_rows(lrmd, ref, torch, inputs, symmetric):
-    """Config 5 at full size, in the launch configuration bench.py times (default: symmetric kernel in 64 launches
-    per force evaluation) and with the ordered kernel: forces on sampled rows (each against all N) at t = 0 and at
+    """Config 5 at full size, in the launch configuration bench.py times (default: the band kernel, one launch per
+    force evaluation) and with the ordered kernel: forces on sampled rows (each against all N) at t = 0 and at
     the GPU's positions after one step."""
     w = inputs.WORKLOADS["grav2d_1m"]
     x, y, px, py = w.state()
     rows = np.random.default_rng(6).choice(w.N, 4096, replace=False)      # SURVEY.md 8(d): >= 4,096 sampled rows
     ctx = lrmd.Context(GRAV2D, w.N, w.eps, options={lrmd.OPT_PAIR_SYMMETRIC: symmetric})
-    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == (1 if symmetric else 0)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == (2 if symmetric else 0)     # default at this N: the band kernel
     ctx.set_state(x, y, px, py)
     fx, fy = (t.cpu().numpy() for t in ctx.forces())
     f0, f1, A0, A1 = ref.forces_rows(GRAV2D, w.eps, x, y, rows, with_abs=True)
