@@ -280,7 +280,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                                 "is context only" % (state_bytes / 1e6))
         elif f32_pairs:
             # fp32 pair arithmetic: one MUFU.RCP per pair on the special-function unit, 16 lanes per SM per clock
-            kernel = "ring_force_f32_kernel" if w.model == 1 else ("grav_force_sym_f32_kernel" if symk else "grav_force_f32_kernel")
+            kernel = "ring_force_f32_kernel" if w.model == 1 else {0: "grav_force_f32_kernel", 1: "grav_force_sym_f32_kernel", 2: "grav_force_band_f32_kernel"}[symk]
             mufu = float(w.N) * float(w.N) * (0.5 if symk else 1.0)      # executed: one per (un)ordered pair evaluated
             peak = SM_COUNT * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
             achieved = mufu / avg_s / 1e12

@@ -82,7 +82,7 @@ enum {
     LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models: force kernels that evaluate every UNORDERED pair once and add +f / -f to
                                     both particles (the paper declines this): 1 = warp-level
                                     kernel (one j-side scratch row per 32R-particle tile; fp64 and, GRAV2D, fp32 pairs),
-                                    2 = band kernel (fp64 only; both sides' sums kept on chip over blocks of 8 x 32R
+                                    2 = band kernel (fp64, and GRAV2D fp32 pairs; both sides' sums kept on chip over blocks of 8 x 32R
                                     particles, one launch for any N, about 25 N doubles of scratch per component);
                                     0 = every ordered pair (the paper's scheme); -1 = choose (1 for 2048 <= N < 49,152,
                                     2 beyond, 0 if the context is a shard).  get: the kernel in use.  With 1

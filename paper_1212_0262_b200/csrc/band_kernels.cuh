@@ -217,6 +217,164 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
     }
 }
 
+// ---- band kernel, fp32 pair terms (rows N1 + N4, GRAV2D) ------------------------------------------------
+// The same blocking on the float2 position stream: the J-block's positions are fp32 (8 bytes per column), the force sums
+// it collects fp64.  A walk's arithmetic is sym_chunk_f32's (2 FADD + 6 FFMA + MUFU.RCP per unordered pair), with the
+// packet in shared memory: per step the lane adds the fp32 sum of its R terms to the slot's fp64 sum (reading G16: fp32
+// sums never run over more than R terms on the j side, 32 on the i side).  64 registers of state per thread instead of
+// the warp-level kernel's 191: 16 resident warps per SM instead of 8.
+template <int R, bool MASK, bool DIAG>
+__device__ __forceinline__ void sym_chunk_f32_smem(const float (&a)[R], const float (&b)[R], const bool (&vi)[R],
+                                                   double (&f0)[R], double (&f1)[R], const float2* __restrict__ spos,
+                                                   double2* __restrict__ sg, int nvalid, float eps) {
+    const int lane = threadIdx.x & 31;
+    float sx[R], sy[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) sx[r] = sy[r] = 0.f;
+    float2 qn = spos[lane];
+#pragma unroll 4
+    for (int s = 0; s < 32; ++s) {
+        const int idx = (lane + s) & 31;
+        const float2 q = qn;
+        qn = spos[(idx + 1) & 31];
+        double2 g = make_double2(0.0, 0.0);
+        if (!DIAG) g = sg[idx];
+        const bool vq = MASK ? (idx < nvalid) : true;
+        float h0 = 0.f, h1 = 0.f;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float dx = a[r] - q.x, dy = b[r] - q.y;
+            const float r2 = fmaf(dy, dy, fmaf(dx, dx, eps));
+            float w = rcp_f32(r2);
+            if (MASK) w = (vi[r] && vq) ? w : 0.f;
+            sx[r] = fmaf(dx, w, sx[r]);
+            sy[r] = fmaf(dy, w, sy[r]);
+            if (!DIAG) {
+                h0 = fmaf(-dx, w, h0);
+                h1 = fmaf(-dy, w, h1);
+            }
+        }
+        if (!DIAG) {
+            sg[idx] = make_double2(g.x + (double)h0, g.y + (double)h1);
+            __syncwarp();
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        f0[r] += (double)sx[r];
+        f1[r] += (double)sy[r];
+    }
+}
+
+constexpr size_t band_f32_smem_bytes(int R) { return (size_t)kBandWarps * 32 * R * (sizeof(float2) + sizeof(double2)) + 16; }
+
+template <int R>
+__global__ void __launch_bounds__(kBandThreads, 2)
+grav_force_band_f32_kernel(const float2* __restrict__ js32, BandPart B, float eps, double pre, double* __restrict__ ibuf0,
+                           double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1) {
+    extern __shared__ __align__(128) unsigned char band_smem[];
+    constexpr int T = 32 * R, IB = kBandWarps * T, JB = IB / 32;
+    double2* Jg = reinterpret_cast<double2*>(band_smem);
+    float2* Jpos = reinterpret_cast<float2*>(Jg + IB);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(Jpos + IB);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long N = B.N;
+    const bool ragged = (N % T) != 0;
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0u;
+
+    const int pfirst = B.wpiece[blockIdx.x], plast = B.wpiece[blockIdx.x + 1];
+    for (int pc = pfirst; pc < plast; ++pc) {
+        const BandPiece piece = B.pieces[pc];
+        const BandInfo band = B.bands[piece.band];
+        const int jbfirst = piece.c0 / JB;
+        for (int jb = jbfirst; jb * JB < piece.c1; ++jb) {
+            const int jc0 = piece.c0 > jb * JB ? piece.c0 : jb * JB;
+            const int jc1 = piece.c1 < (jb + 1) * JB ? piece.c1 : (jb + 1) * JB;
+            const int n = jc1 - jc0;
+            const long long col0 = (long long)jc0 * 32;
+            const int ncol = (int)((N - col0 < (long long)n * 32) ? (N - col0) : (long long)n * 32);
+            const int ncopy = (ncol + 1) & ~1;        // bulk copies move multiples of 16 bytes (the stream is padded by 2)
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                mbar_expect_tx(bar, (uint32_t)ncopy * (uint32_t)sizeof(float2));
+                bulk_g2s(Jpos, js32 + col0, (uint32_t)ncopy * (uint32_t)sizeof(float2), bar);
+            }
+            for (int x = threadIdx.x; x < n * 32; x += kBandThreads) Jg[x] = make_double2(0.0, 0.0);
+            mbar_wait(bar, phase);
+            phase ^= 1u;
+            for (int x = ncol + threadIdx.x; x < n * 32; x += kBandThreads) Jpos[x] = make_float2(0.f, 0.f);
+            __syncthreads();
+
+            const int nv = n >= kBandWarps ? n : kBandWarps;
+            const int off = (warp * nv) / kBandWarps;
+            const int m = nv / kBandWarps;
+            const int blk_end = band.blk0 + band.nblk < jb + 1 ? band.blk0 + band.nblk : jb + 1;
+            for (int b = band.blk0; b < blk_end; ++b) {
+                const bool diag = b == jb;
+                const int tile = b * kBandWarps + warp;
+                const bool tile_any = (long long)tile * T < N;
+                const bool masked_tile = ragged && (long long)(tile + 1) * T > N;
+                float a[R], bb[R];
+                double f0[R], f1[R];
+                bool vi[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const long long i = (long long)tile * T + r * 32 + lane;
+                    vi[r] = i < N;
+                    const float2 q = vi[r] ? js32[i] : make_float2(0.f, 0.f);
+                    a[r] = q.x;
+                    bb[r] = q.y;
+                    f0[r] = 0.0;
+                    f1[r] = 0.0;
+                }
+                for (int k = 0; k < nv; ++k) {
+                    int x = k + off;
+                    if (x >= nv) x -= nv;
+                    if (tile_any && x < n) {
+                        const long long left = N - (long long)(jc0 + x) * 32;
+                        const int nvalid = left < 32 ? (int)left : 32;
+                        const bool masked = masked_tile || nvalid < 32;
+                        const float2* sp = Jpos + x * 32;
+                        double2* sg = Jg + x * 32;
+                        if (diag) {
+                            if (masked) sym_chunk_f32_smem<R, true, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            else sym_chunk_f32_smem<R, false, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                        } else {
+                            if (masked) sym_chunk_f32_smem<R, true, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            else sym_chunk_f32_smem<R, false, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                        }
+                    }
+                    if (!diag && (k + 1) % m == 0 && k + 1 < nv) __syncthreads();
+                }
+                const bool first = jb == (b > jbfirst ? b : jbfirst);
+                const long long rbase = (long long)pc * B.istride - (long long)band.blk0 * IB;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const long long i = (long long)tile * T + r * 32 + lane;
+                    if (vi[r]) {
+                        double v0 = pre * f0[r], v1 = pre * f1[r];
+                        if (!first) { v0 += ibuf0[rbase + i]; v1 += ibuf1[rbase + i]; }
+                        ibuf0[rbase + i] = v0;
+                        ibuf1[rbase + i] = v1;
+                    }
+                }
+                __syncthreads();
+            }
+            const long long jbase = band.joff + col0 - (long long)band.cstart * 32;
+            for (int x = threadIdx.x; x < ncol; x += kBandThreads) {
+                const double2 g = Jg[x];
+                jbuf0[jbase + x] = pre * g.x;
+                jbuf1[jbase + x] = pre * g.y;
+            }
+        }
+    }
+}
+
 // out0 / out1[i] = the force on particle i from one launch of pair_force_band_kernel; then the update (UPD as in
 // pair_sym_fold_kernel).  Block = 32 particles x kFoldGroups term groups; terms of particle i, in this order:
 // the i-side rows of its band's pieces that reached its I-block, then the j-side rows of bands 0 .. its own.

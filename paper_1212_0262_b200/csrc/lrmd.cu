@@ -234,7 +234,8 @@ void resolve_band(lrmd_ctx* c) {
     c->band_infos.clear();
     c->band_owner.clear();
     const int64_t N = c->N;
-    if (c->opt_sym == 0 || c->opt_sym == 1 || c->N_total != c->N || c->opt_precision != 0) return;
+    if (c->opt_sym == 0 || c->opt_sym == 1 || c->N_total != c->N) return;
+    if (c->opt_precision != 0 && c->model != LRMD_GRAV2D) return;     // fp32 pairs: the band kernel exists for 2D only
     if (c->opt_sym < 0 && N < kBandMinN) return;
     const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
     const int64_t IB = (int64_t)kBandWarps * 32 * R, JB = IB / 32;
@@ -807,6 +808,12 @@ void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB 
     double *i0 = wsd(c, c->lay.bibuf0), *i1 = wsd(c, c->lay.bibuf1), *j0 = wsd(c, c->lay.bjbuf0), *j1 = wsd(c, c->lay.bjbuf1);
     const double pre = c->model == LRMD_RING ? -1.0 / (2.0 * std::sqrt(2.0) * (double)c->N) : -2.0 / (double)c->N;
     const dim3 g((unsigned)c->bpart.P), b(kBandThreads);
+    if (c->opt_precision == 1) {
+        L.smem = band_f32_smem_bytes(c->band_R);
+        if (c->band_R == 8) L.go_timed(grav_force_band_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
+        else L.go_timed(grav_force_band_f32_kernel<4>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
+        withv = false;
+    } else {
     L.smem = band_smem_bytes(c->band_R);
 #define LRMD_BAND_GO(M, RR, V) \
     L.go_timed(pair_force_band_kernel<M, RR, V>, g, b, (const double2*)js_ptr(c), c->bpart, c->eps, pre, i0, i1, j0, j1, pre_v, vpart(c))
@@ -818,6 +825,7 @@ void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB 
     }
 #undef LRMD_BAND_V
 #undef LRMD_BAND_GO
+    }
     c->v_valid = withv;
     FusedUpdate U;
     U.q0 = c->a0; U.q1 = nullptr; U.p0 = c->a1; U.p1 = nullptr;

@@ -168,3 +168,36 @@ def test_band_step_observe_uses_the_fused_potential(lrmd, ref, torch, model, N, 
     # per record after the first: the kinetic partial kernel and the finalize kernel only (no pair sweep); the first
     # record takes the separate sweep (pack? no: + kinetic, energy kernel, finalize)
     assert launches - plain <= 3 + 3 * 2 + 2
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 255, 1023, 2049, 4099, 20_011])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_band_f32_pair_variant_forces(lrmd, ref, torch, N, variant):
+    """GRAV2D, fp32 pair terms in the band kernel: 1e-5 A_i, odd N (the fp32 stream's bulk copies move an
+    even number of elements), any number of workers and band heights; bitwise reproducible."""
+    st = _state(GRAV2D, N, 950 + N % 13)
+    f0, f1, A0, A1 = ref.forces_abs(GRAV2D, 1e-3, st[0], st[1], form=0)
+    for workers, height in ((0, 0), (3, 1), (37, 2)):
+        opts = {lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_VARIANT: variant,
+                lrmd.OPT_PAIR_CTAS: workers, lrmd.OPT_PAIR_BAND_HEIGHT: height}
+        got = _forces(lrmd, GRAV2D, N, 1e-3, st, opts)
+        again = _forces(lrmd, GRAV2D, N, 1e-3, st, opts)
+        for g, h, w, a in ((got[0], again[0], f0, A0), (got[1], again[1], f1, A1)):
+            assert np.array_equal(g, h)
+            err = np.abs(g - w)
+            assert np.all(err <= 1e-5 * a + 1e-300), float((err / np.maximum(a, 1e-300)).max())
+
+
+def test_band_f32_pair_variant_trajectory(lrmd, ref, torch):
+    N = 70_001          # default choice at this size with fp32 pairs: the band kernel
+    st = _state(GRAV2D, N, 24)
+    ctx = lrmd.Context(GRAV2D, N, 1e-3, options={lrmd.OPT_PAIR_PRECISION: 1})
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    ctx.set_state(*st)
+    ctx.step(3, 0.005)
+    got = ctx.state_numpy()
+    ctx.close()
+    r = [a.copy() for a in st]
+    ref.step(GRAV2D, 1e-3, r[0], r[1], r[2], r[3], 3, 0.005, form=1)
+    for g, w in zip(got, r):
+        assert np.max(np.abs(g - w)) <= 1e-6

@@ -595,8 +595,11 @@ def test_symmetric_default_choice(lrmd, torch):
     assert c.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2 and c.get_option(lrmd.OPT_PAIR_FUSE_UPDATE) == 1
     assert b1.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1
     assert b1.get_option(lrmd.OPT_PAIR_SYM_TILES) == 256    # all 256 tiles in one launch (268 MB of j-side rows)
-    # fp32 pair arithmetic has no band kernel: warp-level kernel, 64 launches of 64 tiles at N = 2^20
-    assert c1.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and c1.get_option(lrmd.OPT_PAIR_SYM_TILES) == 64
+    # fp32 pair arithmetic (2D) has its own band kernel; the warp-level one would take 64 launches of 64 tiles here
+    assert c1.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    c2 = lrmd.Context(GRAV2D, 1_048_576, 1e-3, options={lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_SYMMETRIC: 1})
+    assert c2.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 1 and c2.get_option(lrmd.OPT_PAIR_SYM_TILES) == 64
+    c2.close()
     assert d.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0 and e.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 0
     for x in (a, b, c, d, e, b1, c1):
         x.close()
