@@ -188,7 +188,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     stream = torch.cuda.current_stream(dev)
     state_bytes = ctx.narrays * w.N * 8
     larger_than_l2 = state_bytes > L2_BYTES
-    resident_by_design = w.key == "hmf_1e4"
+    resident_by_design = w.model == 0 and ctx.get_option(lrmd.OPT_HMF_VARIANT) in (3, 4)
     flush = None
     if not larger_than_l2 and not resident_by_design:
         flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
@@ -264,18 +264,21 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         clk = (clocks.get("sm_mhz") or peaks["sm_max_mhz"])
         symk = ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) if w.model != 0 else 0     # 0 ordered, 1 warp-level, 2 band
         if w.model == 0:
-            kernel = {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel"}.get(ctx.get_option(lrmd.OPT_HMF_VARIANT),
-                                                                             "hmf_substage_tma_kernel")
+            kernel = {0: "hmf_substage_kernel", 3: "hmf_cluster_kernel", 4: "hmf_grid_kernel"}.get(
+                ctx.get_option(lrmd.OPT_HMF_VARIANT), "hmf_substage_tma_kernel")
             bytes_per_launch = HMF_BYTES_PER_PARTICLE_SUBSTAGE * w.N
-            if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 3:
-                # cluster-resident kernel: one launch runs all Kr steps with the state in registers; the figure is
+            if ctx.get_option(lrmd.OPT_HMF_VARIANT) in (3, 4):
+                # cluster- / grid-resident kernels: one launch runs all Kr steps with the state on chip; the figure is
                 # what the same substages would stream through HBM (context only: the working set is on chip)
                 bytes_per_launch *= 3.0 * Kr
             achieved = bytes_per_launch / avg_s / 1e9
             roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "frac": achieved / peaks["hbm_gbs"], "peak_source": peaks["source"] + " (MEASURED_PEAKS.json hbm_gbs)",
                     "algorithmic_bytes_per_launch": bytes_per_launch}
-            if 2.0 * state_bytes <= L2_BYTES:
+            if ctx.get_option(lrmd.OPT_HMF_VARIANT) == 4:
+                roof["note"] = ("grid-resident kernel: the state (%.1f MB) stays in shared memory for the whole call; the step is bound by "
+                                "the grid barrier between substages, the HBM figure is context only" % (state_bytes / 1e6))
+            elif 2.0 * state_bytes <= L2_BYTES:
                 roof["note"] = ("state (%.1f MB) fits the 126 MB L2: the substages stream it through L2, not HBM; the HBM figure "
                                 "is context only" % (state_bytes / 1e6))
         elif f32_pairs:
@@ -424,8 +427,9 @@ def l2_statement(w):
     state_bytes = narr * w.N * 8
     if state_bytes > L2_BYTES:
         return "inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)
-    if w.key == "hmf_1e4":
-        return "not flushed: %.2f MB working set is on-chip by design, latency-bound case" % (state_bytes / 1e6)
+    if w.model == 0 and w.N < 1_000_000:
+        return ("not flushed: the %.2f MB state stays on chip (registers of one cluster / shared memory of the grid) for all "
+                "steps of the one launch, by design; latency-bound case" % (state_bytes / 1e6))
     return "L2 flushed (256 MiB write) before every timed step"
 
 

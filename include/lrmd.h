@@ -75,7 +75,11 @@ enum {
                                     replay off while set.  Measurement aid: results are unchanged.          */
     LRMD_OPT_HMF_VARIANT = 5,    /* HMF: 0 = register-prefetch substage kernel, 1-2 = TMA-staged substage kernel
                                     shapes, 3 = cluster-resident kernel (N <= 20,480: state in registers of one
-                                    thread-block cluster, all n steps of a call in one launch); -1 = choose from N */
+                                    thread-block cluster, all n steps of a call in one launch), 4 = grid-resident kernel
+                                    (N <= 1,070,336: state in the shared memory of one CTA per SM, all n steps of a call
+                                    in one cooperative launch, a grid barrier per substage; falls back to 0 if the device
+                                    refuses the cooperative launch); -1 = choose from N (3 up to 20,480, 4 up to 1,070,336,
+                                    1 beyond; shards: 0 below 1e6, else 1)                                                  */
     LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
                                     of the pair kernels (-1 = choose)                                          */
     LRMD_OPT_PAIR_SLOTS = 7,     /* read-only (lrmd_get_option): partial force rows per particle          */

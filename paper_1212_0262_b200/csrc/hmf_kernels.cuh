@@ -16,6 +16,8 @@
 // fences) — all CTAs therefore get bit-identical (Mx, My).
 #pragma once
 
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 #include "trig.cuh"
 
@@ -424,6 +426,118 @@ hmf_cluster_kernel(double* __restrict__ theta, double* __restrict__ p, long long
     }
     // the sums at the final angles, for lrmd_forces / lrmd_energy / the next call (reading G3)
     if (rank == 0 && tid < C) partial_out[tid] = cta_part[parity ^ 1][tid];
+}
+
+// ---- grid-resident variant (20,480 < N < 1e6: the paper's Table 1 sizes 1e5 .. 1e6) ----------------
+// Between the cluster-resident kernel and the HBM regime the state (16 N bytes) fits the GPU's shared memory, and a
+// substage's arithmetic takes 0.2 - 2 us: what a step costs is the kernel boundary between substages (7.7 us each with
+// a replayed CUDA graph).  One cooperative launch of one CTA per SM keeps the whole state — angles, momenta and the
+// sin / cos of the current angles — in shared memory and runs ALL n steps of an lrmd_step call; a substage is one
+// pass over the CTA's particles (kick, drift, sincos, partial sums), a block reduction, the CTA's (sum cos, sum sin)
+// written to a double-buffered array in global memory, a grid barrier (cooperative groups grid.sync(); a hand-written
+// all-gather on per-CTA flag words measured 7.5 us per substage against 3.1 us and was dropped), and a fixed tree over
+// the G partials that every CTA evaluates identically.  Deterministic: fixed particle -> CTA -> thread map, fixed trees.
+constexpr int kHmfGridThreads = 512;
+constexpr int kHmfGridBytesPerParticle = 32;                        // theta, p, sin, cos
+constexpr int kHmfGridMaxLocal = (227 * 1024 - 1024) / kHmfGridBytesPerParticle;   // particles per CTA that fit
+
+__global__ void __launch_bounds__(kHmfGridThreads, 1)
+hmf_grid_kernel(double* __restrict__ theta, double* __restrict__ p, long long N, int nlocal, long long nsteps, double kB0,
+                double kB1, double dD0, double dD1, double2* __restrict__ part2, double2* __restrict__ partial_out) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    extern __shared__ __align__(16) unsigned char hmf_grid_smem[];
+    constexpr int T = kHmfGridThreads, NW = T / 32;
+    __shared__ double scratch[2 * NW];
+    __shared__ double2 wtot[8];
+    double* th = reinterpret_cast<double*>(hmf_grid_smem);
+    double* pp = th + nlocal;
+    double* sn = pp + nlocal;
+    double* cs = sn + nlocal;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int G = (int)gridDim.x;
+    const long long i0 = (long long)blockIdx.x * nlocal;
+    const int n = (int)((N - i0 < nlocal) ? (N - i0 > 0 ? N - i0 : 0) : nlocal);
+    const double inv_n = 1.0 / (double)N;
+    for (int k = tid; k < n; k += T) {
+        th[k] = theta[i0 + k];
+        pp[k] = p[i0 + k];
+    }
+    __syncthreads();
+
+    int parity = 0;
+    double Mx = 0.0, My = 0.0;
+    // One substage: [kick kA (+ kB)] -> [drift] -> sincos -> (Mx, My).  KICK = 0: the first reduction of the call.
+    auto pass = [&](int kicks, double kA, double kB, double dc) {
+        double aC = 0.0, aS = 0.0;
+        for (int k = tid; k < n; k += T) {
+            double x = th[k];
+            if (kicks > 0) {
+                const double f = fma(cs[k], My, -(sn[k] * Mx));
+                double q = fma(kA, f, pp[k]);
+                if (kicks > 1) q = fma(kB, f, q);
+                pp[k] = q;
+                x = fma(dc, q, x);
+                th[k] = x;
+            }
+            double s, c;
+            sincos_any(x, s, c);
+            sn[k] = s;
+            cs[k] = c;
+            aC += c;
+            aS += s;
+        }
+        double r[2] = {aC, aS};
+        block_sum<T, 2>(r, scratch);
+        if (tid == 0) {
+            __stcg(reinterpret_cast<double*>(&part2[(size_t)parity * G + blockIdx.x]), r[0]);
+            __stcg(reinterpret_cast<double*>(&part2[(size_t)parity * G + blockIdx.x]) + 1, r[1]);
+        }
+        grid.sync();
+        // the same tree in every CTA: thread t < G takes partial t; xor-shuffle trees in warps 0 .. 7, then in order
+        double qx = 0.0, qy = 0.0;
+        if (tid < G) {
+            qx = __ldcg(reinterpret_cast<const double*>(&part2[(size_t)parity * G + tid]));
+            qy = __ldcg(reinterpret_cast<const double*>(&part2[(size_t)parity * G + tid]) + 1);
+        }
+        if (w < 8) {
+            qx = warp_sum(qx);
+            qy = warp_sum(qy);
+            if (lane == 0) wtot[w] = make_double2(qx, qy);
+        }
+        __syncthreads();
+        double sC = 0.0, sS = 0.0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            sC += wtot[k].x;
+            sS += wtot[k].y;
+        }
+        Mx = sC * inv_n;
+        My = sS * inv_n;
+        parity ^= 1;
+        __syncthreads();      // wtot is rewritten by the next pass
+    };
+
+    pass(0, 0.0, 0.0, 0.0);                          // f(q(t)): listing step 1
+    for (long long s = 0; s < nsteps; ++s) {         // listing steps 2-11, readings G2-G4
+        // the closing kick B0 of the previous step and this step's opening kick: two FMAs with the same force
+        if (s == 0) pass(1, kB0, 0.0, dD0);
+        else pass(2, kB0, kB0, dD0);
+        pass(1, kB1, 0.0, dD1);
+        pass(1, kB1, 0.0, dD0);
+    }
+    for (int k = tid; k < n; k += T) {
+        double q = pp[k];
+        if (nsteps > 0) q = fma(kB0, fma(cs[k], My, -(sn[k] * Mx)), q);      // closing kick of the last step
+        theta[i0 + k] = th[k];
+        p[i0 + k] = q;
+    }
+    // the per-CTA sums at the final angles, for lrmd_forces / lrmd_energy / the next call (reading G3)
+    if (blockIdx.x == 0 && tid < G) {
+        const double2 v = make_double2(__ldcg(reinterpret_cast<const double*>(&part2[(size_t)(parity ^ 1) * G + tid])),
+                                       __ldcg(reinterpret_cast<const double*>(&part2[(size_t)(parity ^ 1) * G + tid]) + 1));
+        partial_out[tid] = v;
+    }
 }
 
 // Sharded runs ("each GPU computes its contribution to the magnetisation, which are then summed"):

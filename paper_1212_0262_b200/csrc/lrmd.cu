@@ -78,6 +78,7 @@ struct lrmd_ctx {
     int band_R = 8;
     size_t band_jrow = 0;       // elements of all bands' j-side rows
     bool use_graph = false;
+    bool grid_unavailable = false;   // a cooperative launch of the grid-resident HMF kernel failed: not tried again
     Layout lay;
     // bindings
     char* ws = nullptr;
@@ -112,8 +113,10 @@ namespace {
 // HMF: variant 0 is the register-prefetch kernel, 1-2 the TMA-staged kernel <consumer threads, stages, CTAs per
 // SM> (N >= 1e6), 3 the cluster-resident kernel (N <= 20,480: the step is latency-bound).
 struct HmfVariant { int consumers, stages, minb; };
-constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}, {-1, 0, 0}};
+constexpr HmfVariant kHmfVariants[] = {{0, 0, 0}, {512, 4, 1}, {256, 6, 2}, {-1, 0, 0}, {-2, 0, 0}};
 constexpr int kHmfClusterVariant = 3;   // cluster-resident kernel: whole state in registers, all steps in one launch
+constexpr int kHmfGridVariant = 4;      // grid-resident kernel: whole state in shared memory, one cooperative launch per call
+constexpr int64_t kHmfGridMaxN = (int64_t)kNumSm * kHmfGridMaxLocal;   // 1,070,336
 constexpr int64_t kHmfClusterMaxN = (int64_t)kHmfClusterCtas * kHmfClusterThreads * 8;   // 20,480
 constexpr int kNumHmfVariants = sizeof(kHmfVariants) / sizeof(kHmfVariants[0]);
 constexpr int64_t kHmfTmaMinN = 1000000;
@@ -346,11 +349,17 @@ void resolve(lrmd_ctx* c) {
     if (c->model == LRMD_HMF) {
         const bool sharded = c->N_total != c->N;
         c->hmf_variant = c->opt_hmf_variant >= 0 ? (int)c->opt_hmf_variant
-                         : (N >= kHmfTmaMinN ? 1 : (N <= kHmfClusterMaxN ? kHmfClusterVariant : 0));
+                         : (N <= kHmfClusterMaxN ? kHmfClusterVariant
+                            : ((N <= kHmfGridMaxN && !sharded && !c->grid_unavailable) ? kHmfGridVariant
+                               : (N >= kHmfTmaMinN ? 1 : 0)));
         if (c->hmf_variant == kHmfClusterVariant && (N > kHmfClusterMaxN || sharded)) c->hmf_variant = 0;
+        if (c->hmf_variant == kHmfGridVariant && (N > kHmfGridMaxN || sharded || c->grid_unavailable))
+            c->hmf_variant = N >= kHmfTmaMinN ? 1 : 0;
         const HmfVariant hv = kHmfVariants[c->hmf_variant];
         int64_t g;
-        if (c->hmf_variant == kHmfClusterVariant) {
+        if (c->hmf_variant == kHmfGridVariant) {
+            g = kNumSm;        // one CTA per SM; the other HMF kernels read this many partials
+        } else if (c->hmf_variant == kHmfClusterVariant) {
             // the other HMF kernels of this context (forces, energy) read this many partials
             g = c->opt_hmf_grid == kHmfClusterCtasMax ? kHmfClusterCtasMax : kHmfClusterCtas;
         } else if (c->hmf_variant == 0) {
@@ -368,7 +377,7 @@ void resolve(lrmd_ctx* c) {
         c->slots = 1;
         L.hmf_partial = off; off = align_up(off + 3 * sizeof(double2) * kHmfMaxGrid);
         c->use_graph = c->opt_graph < 0 ? (N <= (1 << 20)) : (c->opt_graph != 0);
-        if (c->hmf_variant == kHmfClusterVariant || sharded) c->use_graph = false;   // collectives between substages
+        if (c->hmf_variant == kHmfClusterVariant || c->hmf_variant == kHmfGridVariant || sharded) c->use_graph = false;   // (collectives between substages)
         L.shared2 = off; off = align_up(off + sizeof(double2));
     } else {
         c->pair_variant = c->opt_pair_variant >= 0 ? (int)c->opt_pair_variant : (c->model == LRMD_GRAV2D ? 1 : 0);
@@ -696,8 +705,63 @@ int hmf_step_cluster(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     return LRMD_OK;
 }
 
+// All n steps in one cooperative launch of one CTA per SM (hmf_grid_kernel).  Returns LRMD_EUNSUPPORTED if the device
+// refuses the cooperative launch (the caller then falls back to the substage kernels).
+int hmf_step_grid(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
+    const Coef k = coefficients();
+    const int G = c->hmf_grid;
+    const int nlocal = (int)((c->N + G - 1) / G);
+    const size_t smem = (size_t)nlocal * kHmfGridBytesPerParticle;
+    bool ready = false;
+    for (const void* f : c->smem_ready) ready = ready || f == (const void*)hmf_grid_kernel;
+    if (!ready) {
+        const cudaError_t ea = cudaFuncSetAttribute((const void*)hmf_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                    (int)((size_t)kHmfGridMaxLocal * kHmfGridBytesPerParticle));
+        if (ea != cudaSuccess) { c->cuda_err = (int)ea; (void)cudaGetLastError(); return LRMD_EUNSUPPORTED; }
+        c->smem_ready.push_back((const void*)hmf_grid_kernel);
+    }
+    cudaLaunchConfig_t cfg;
+    std::memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(G);
+    cfg.blockDim = dim3(kHmfGridThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const bool t = c->timing && c->ev_used + 2 <= kMaxTimedEvents;
+    if (t) {
+        while (c->ev.size() < c->ev_used + 2) {
+            cudaEvent_t e;
+            const cudaError_t ee = cudaEventCreate(&e);
+            if (ee != cudaSuccess) { c->cuda_err = (int)ee; (void)cudaGetLastError(); return LRMD_ECUDA; }
+            c->ev.push_back(e);
+        }
+        cudaEventRecord(c->ev[c->ev_used], stream);
+    }
+    const int nxt = (c->cur + 1) % 3;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, hmf_grid_kernel, c->a0, c->a1, (long long)c->N, nlocal, (long long)n,
+                                             k.B0 * dt, k.B1 * dt, k.D0 * dt, k.D1 * dt, hmf_buf(c, nxt), hmf_buf(c, c->cur));
+    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_EUNSUPPORTED; }
+    if (t) { cudaEventRecord(c->ev[c->ev_used + 1], stream); c->ev_used += 2; }
+    ++c->launches;
+    c->force_valid = true;   // the kernel leaves the per-CTA sums at the final angles in the current partial buffer
+    return LRMD_OK;
+}
+
 int hmf_step(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     if (c->hmf_variant == kHmfClusterVariant) return hmf_step_cluster(c, n, dt, stream);
+    if (c->hmf_variant == kHmfGridVariant) {
+        const int rc = hmf_step_grid(c, n, dt, stream);
+        if (rc != LRMD_EUNSUPPORTED) return rc;
+        // the device does not grant the cooperative launch (fewer SMs available than CTAs): substage kernels instead
+        c->grid_unavailable = true;
+        resolve(c);
+        drop_graph(c);
+        c->force_valid = false;
+    }
     const Coef k = coefficients();
     Launcher L{c, stream};
     if (!c->force_valid) { hmf_reduce_only(L); c->force_valid = true; }

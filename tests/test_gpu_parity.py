@@ -183,6 +183,49 @@ def test_hmf_cluster_variant_falls_back_above_its_size(lrmd, torch):
     ctx.close()
 
 
+@pytest.mark.parametrize("N", [1, 2, 147, 149, 20_481, 100_000, 300_001, 1_070_336])
+def test_hmf_grid_resident_kernel_matches_oracle(lrmd, ref, torch, N):
+    """LRMD_OPT_HMF_VARIANT = 4: the whole state in shared memory, one cooperative launch per lrmd_step call, a grid
+    barrier per substage.  Fewer particles than CTAs, ragged shares, the largest size that fits; forces before and
+    after, 10-step trajectory, energies; step(10) == 10 x step(1) bit for bit; run-to-run reproducible."""
+    st = _state(HMF, N, 2_000 + N % 11)
+    outs = []
+    for single in (False, True, False):
+        ctx = lrmd.Context(HMF, N, 0.0, options={lrmd.OPT_HMF_VARIANT: 4})
+        assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == 4
+        ctx.set_state(*st)
+        if single:
+            for _ in range(10):
+                ctx.step(1, 0.05)
+        else:
+            ctx.step(10, 0.05)
+        outs.append(ctx.state_numpy())
+        f = ctx.forces().cpu().numpy()
+        e = ctx.energy().cpu().numpy()
+        assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == 4          # no fallback happened
+        ctx.close()
+    for other in outs[1:]:
+        assert np.array_equal(outs[0][0], other[0]) and np.array_equal(outs[0][1], other[1])
+    th, p = st[0].copy(), st[1].copy()
+    ref.step(HMF, 0.0, th, None, p, None, 10, 0.05, form=0)
+    assert np.max(np.abs(outs[0][0] - th)) <= XTOL and np.max(np.abs(outs[0][1] - p)) <= XTOL
+    f1, _, S1, _ = ref.forces_abs(HMF, 0.0, outs[0][0], None, form=0)
+    assert np.all(np.abs(f - f1) <= FTOL * S1 + 4e-16)
+    er, ea = ref.energy(HMF, 0.0, outs[0][0], None, outs[0][1], None)
+    assert abs(e[0] - er[0]) <= 1e-12 * max(ea[0], 1e-300) and abs(e[1] - er[1]) <= 1e-12 * max(ea[1], 0.5 * N)
+
+
+def test_hmf_grid_resident_kernel_default_range_and_limits(lrmd, torch):
+    a = lrmd.Context(HMF, 20_480, 0.0)
+    b = lrmd.Context(HMF, 20_481, 0.0)
+    c = lrmd.Context(HMF, 1_000_000, 0.0)
+    d = lrmd.Context(HMF, 1_070_337, 0.0, options={lrmd.OPT_HMF_VARIANT: 4})      # does not fit: TMA-staged kernel
+    assert a.get_option(lrmd.OPT_HMF_VARIANT) == 3 and b.get_option(lrmd.OPT_HMF_VARIANT) == 4
+    assert c.get_option(lrmd.OPT_HMF_VARIANT) == 4 and d.get_option(lrmd.OPT_HMF_VARIANT) == 1
+    for x in (a, b, c, d):
+        x.close()
+
+
 @pytest.mark.parametrize("variant", [1, 2])
 def test_hmf_tma_variant_graph_and_grid(lrmd, torch, variant):
     """Graph replay and a non-default grid give the same bits as plain launches of the same variant and grid."""
@@ -480,15 +523,15 @@ def test_pair_default_path_switch(lrmd, ref, torch, model, N):
         assert np.max(np.abs(g - w)) <= XTOL
 
 
-@pytest.mark.parametrize("N", [999_999, 1_000_000, 1_000_001])
+@pytest.mark.parametrize("N", [1_070_335, 1_070_336, 1_070_337])
 def test_hmf_default_path_switch(lrmd, ref, torch, N):
-    """Either side of the HMF default-kernel switch at N = 1e6 (graph-replayed register-prefetch kernel below,
-    TMA-staged persistent kernel from there), default options: forces at t = 0, a 10-step trajectory (9 steady
+    """Either side of the HMF default-kernel switch at N = 1,070,336 = 148 x 7232 (grid-resident kernel while the state
+    fits the shared memory of one CTA per SM, TMA-staged persistent kernel beyond), default options: forces at t = 0, a 10-step trajectory (9 steady
     steps: one graph replay of 8 below the switch), forces and energies at the end, against the oracle."""
     st = _state(HMF, N, 1_000 + N % 7)
     ctx = lrmd.Context(HMF, N, 0.0)
-    assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == (1 if N >= 1_000_000 else 0)
-    assert ctx.get_option(lrmd.OPT_GRAPH) == (1 if N <= (1 << 20) else 0)
+    assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == (1 if N > 1_070_336 else 4)
+    assert ctx.get_option(lrmd.OPT_GRAPH) == 0
     ctx.set_state(*st)
     f = ctx.forces().cpu().numpy()
     f0, _, S0, _ = ref.forces_abs(HMF, 0.0, st[0], None, form=0)
