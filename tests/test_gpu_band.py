@@ -201,3 +201,19 @@ def test_band_f32_pair_variant_trajectory(lrmd, ref, torch):
     ref.step(GRAV2D, 1e-3, r[0], r[1], r[2], r[3], 3, 0.005, form=1)
     for g, w in zip(got, r):
         assert np.max(np.abs(g - w)) <= 1e-6
+
+
+def test_band_fused_potential_at_config3_size(lrmd, ref, torch, inputs):
+    """Config 3 (N = 65,536) in the default configuration: the V that the step's last force evaluation delivers
+    (lrmd_step_observe) against the oracle's pair sum at the GPU's own final state, and against the separate sweep."""
+    w = inputs.WORKLOADS["grav2d_64k"]
+    ctx = lrmd.Context(GRAV2D, w.N, w.eps)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    ctx.set_state(*w.state())
+    rec = ctx.step_observe(2, w.dt, 1).cpu().numpy()
+    x, y, px, py = ctx.state_numpy()
+    sweep = ctx.energy().cpu().numpy()
+    ctx.close()
+    er, ea = ref.energy(GRAV2D, w.eps, x, y, px, py)
+    assert abs(rec[2, 0] - er[0]) <= 1e-12 * ea[0] and abs(rec[2, 1] - er[1]) <= 1e-12 * ea[1]
+    assert abs(sweep[1] - er[1]) <= 1e-12 * ea[1] and abs(sweep[1] - rec[2, 1]) <= 1e-12 * ea[1]
