@@ -78,7 +78,7 @@ def ncu_traffic(entry, kernel):
 
 
 DEFAULT_STEPS = {"hmf_1e4": 1000, "ring_16k": 100, "grav2d_64k": 50, "hmf_5e7": 100, "grav2d_1m": 5,
-                 "hmf_1e5": 1000, "hmf_1e6": 500, "hmf_1e7": 200}
+                 "hmf_1e5": 1000, "hmf_1e6": 500, "hmf_1e7": 200, "ring_102k": 10, "ring_512k": 3, "grav2d_102k": 10}
 
 
 def measured_peaks():
@@ -613,7 +613,7 @@ def main():
         return 0
 
     from paper_1212_0262_b200 import inputs
-    all_workloads = dict(inputs.WORKLOADS, **inputs.TABLE1_WORKLOADS)
+    all_workloads = dict(inputs.WORKLOADS, **inputs.TABLE1_WORKLOADS, **inputs.TABLE23_WORKLOADS)
     w = all_workloads[args.workload]
     if args.impl == "reference":
         args.steps = args.steps or 3
@@ -682,6 +682,13 @@ def main():
         for key, ow in inputs.TABLE1_WORKLOADS.items():
             if key != w.key:
                 add(key, ow, DEFAULT_STEPS[key], with_e2e=False)
+        # pair-model sizes of the paper's Tables 2 and 3 beyond the configs
+        for key, ow in inputs.TABLE23_WORKLOADS.items():
+            if key != w.key:
+                add(key, ow, DEFAULT_STEPS[key], with_e2e=False, roofline_steps=3)
+        for key, sec in inputs.PAPER_SECONDS_PER_STEP.items():
+            if key in others:
+                others[key]["paper_seconds_per_step_one_gk104"] = sec      # PAPER.md Tables 1-3: context, other hardware
         # the paper's own scheme, every ORDERED pair, on the configs where a symmetric kernel is the default
         for key in ("ring_16k", "grav2d_64k", "grav2d_1m"):
             steps = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]

@@ -268,8 +268,11 @@ __device__ __forceinline__ void sym_chunk_f32_smem(const float (&a)[R], const fl
 
 constexpr size_t band_f32_smem_bytes(int R) { return (size_t)kBandWarps * 32 * R * (sizeof(float2) + sizeof(double2)) + 16; }
 
+// (R = 16, launch shape 2: 255 registers, one CTA per SM; 3.5 % faster than R = 8 at N = 102,400, not the default.
+//  Packed fp32x2 arithmetic (FADD2 / FFMA2) was tried for the walk and measured 5 % slower: the packed instructions
+//  issue at half rate and the pair packing costs register moves.)
 template <int R>
-__global__ void __launch_bounds__(kBandThreads, 2)
+__global__ void __launch_bounds__(kBandThreads, (R <= 8 ? 2 : 1))
 grav_force_band_f32_kernel(const float2* __restrict__ js32, BandPart B, float eps, double pre, double* __restrict__ ibuf0,
                            double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1) {
     extern __shared__ __align__(128) unsigned char band_smem[];

@@ -240,11 +240,13 @@ void resolve_band(lrmd_ctx* c) {
     if (c->opt_sym == 0 || c->opt_sym == 1 || c->N_total != c->N) return;
     if (c->opt_precision != 0 && c->model != LRMD_GRAV2D) return;     // fp32 pairs: the band kernel exists for 2D only
     if (c->opt_sym < 0 && N < kBandMinN) return;
-    const int R = c->opt_pair_variant == 0 ? 4 : (c->opt_pair_variant == 1 ? 8 : (c->model == LRMD_RING ? 4 : 8));
+    // rows per lane: 8 for both models (Ring measured 7.7 % faster than with 4 at N = 512,000); launch shape 0 asks for 4
+    int R = c->opt_pair_variant == 0 ? 4 : 8;
+    if (c->opt_precision == 1 && c->opt_pair_variant == 2) R = 16;      // fp32 pairs: experimental 16 rows per lane
     const int64_t IB = (int64_t)kBandWarps * 32 * R, JB = IB / 32;
     const int64_t nIB = (N + IB - 1) / IB, nchunks = (N + 31) / 32;
     if (nIB > (1 << 20)) return;
-    const int64_t P = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : 2 * (int64_t)kNumSm;
+    const int64_t P = c->opt_pair_ctas > 0 ? c->opt_pair_ctas : (R == 16 ? 1 : 2) * (int64_t)kNumSm;
     // band height: the i-side rows cost (pieces ~ P + bands) x hb x IB elements, the j-side rows ~ bands x N / 2.  A CTA
     // adds to its piece's i-side row once per (J-block, I-block) visit, cycling through hb x IB rows: the height is
     // capped so that the rows all CTAs cycle through stay in L2 (kBandL2Bytes of the 126 MB), else every visit would
@@ -874,7 +876,8 @@ void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB 
     const dim3 g((unsigned)c->bpart.P), b(kBandThreads);
     if (c->opt_precision == 1) {
         L.smem = band_f32_smem_bytes(c->band_R);
-        if (c->band_R == 8) L.go_timed(grav_force_band_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
+        if (c->band_R == 16) L.go_timed(grav_force_band_f32_kernel<16>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
+        else if (c->band_R == 8) L.go_timed(grav_force_band_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
         else L.go_timed(grav_force_band_f32_kernel<4>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
         withv = false;
     } else {

@@ -119,3 +119,14 @@ TABLE1_WORKLOADS = {
     "hmf_1e6": Workload("hmf_1e6", 7, HMF, 1_000_000, 0.0, 0.05, 500, theta_hw=1.5, p_hw=0.5),
     "hmf_1e7": Workload("hmf_1e7", 8, HMF, 10_000_000, 0.0, 0.05, 200, theta_hw=1.5, p_hw=0.5),
 }
+
+# Pair-model sizes of the paper's Tables 2 and 3 beyond BASELINE.json's configs: the largest Ring
+# run (N = 512,000) and the N = 102,400 rows of both tables; same distributions as configs 2 and 3, own seeds.
+TABLE23_WORKLOADS = {
+    "ring_102k": Workload("ring_102k", 9, RING, 102_400, 0.01, 0.01, 10, theta_hw=1.0, p_hw=0.3),
+    "ring_512k": Workload("ring_512k", 10, RING, 512_000, 0.01, 0.01, 3, theta_hw=1.0, p_hw=0.3),
+    "grav2d_102k": Workload("grav2d_102k", 11, GRAV2D, 102_400, 1e-3, 0.005, 10, sigma_p=0.1),
+}
+# seconds per time step the paper reports on one GK104 of a GTX 690 (Tables 1-3; context only, other hardware)
+PAPER_SECONDS_PER_STEP = {"hmf_1e5": 6.3e-4, "hmf_1e6": 4.0e-3, "hmf_1e7": 3.7e-2, "hmf_5e7": 1.81e-1,
+                          "ring_102k": 3.9, "ring_512k": 97.5, "grav2d_102k": 0.99}

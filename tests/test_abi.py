@@ -347,7 +347,7 @@ def test_band_partition_covers_every_column_once_and_is_balanced(lrmd, model, N,
     rc, tab = lrmd.lrmd_pair_band_partition(h)
     assert rc == lrmd.OK and len(tab) >= 1
     IB, P = int(tab[0, 6]), int(tab[0, 7])
-    R = 4 if (variant == 0 or (variant < 0 and model == RING)) else 8
+    R = 4 if variant == 0 else 8           # 8 rows per lane by default, for both models
     assert IB == 8 * 32 * R and P == (workers or 296)
     JB = IB // 32
     nIB, nchunks = -(-N // IB), -(-N // 32)

@@ -40,7 +40,7 @@ def test_band_force_kernel_matches_oracle(lrmd, ref, torch, model, N, variant):
 
 @pytest.mark.parametrize("model", [RING, GRAV2D])
 def test_band_kernel_default_shape_several_bands(lrmd, ref, torch, model):
-    """N = 70,001: beyond the default switch (49,152), 35 (2D) / 69 (Ring) I-blocks, default band height and workers;
+    """N = 70,001: beyond the default switch (49,152), 35 I-blocks of 2048 rows, default band height and workers;
     forces on sampled rows against the oracle (each against all N)."""
     eps = _eps(model)
     N = 70_001
@@ -171,7 +171,7 @@ def test_band_step_observe_uses_the_fused_potential(lrmd, ref, torch, model, N, 
 
 
 @pytest.mark.parametrize("N", [1, 2, 3, 255, 1023, 2049, 4099, 20_011])
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_band_f32_pair_variant_forces(lrmd, ref, torch, N, variant):
     """GRAV2D, fp32 pair terms in the band kernel: 1e-5 A_i, odd N (the fp32 stream's bulk copies move an
     even number of elements), any number of workers and band heights; bitwise reproducible."""
@@ -217,3 +217,24 @@ def test_band_fused_potential_at_config3_size(lrmd, ref, torch, inputs):
     er, ea = ref.energy(GRAV2D, w.eps, x, y, px, py)
     assert abs(rec[2, 0] - er[0]) <= 1e-12 * ea[0] and abs(rec[2, 1] - er[1]) <= 1e-12 * ea[1]
     assert abs(sweep[1] - er[1]) <= 1e-12 * ea[1] and abs(sweep[1] - rec[2, 1]) <= 1e-12 * ea[1]
+
+
+def test_ring_512k_paper_table2_size_sampled_rows(lrmd, ref, torch, inputs):
+    """The largest Ring run of the paper's Table 2 (N = 512,000) in the default configuration (band
+    kernel, I-blocks of 2048 rows): forces on 2,048 sampled rows, each against all N, against the oracle's direct
+    eq.(8) form; K and V after one step against the oracle at the GPU's own state on the same rows' scale."""
+    w = inputs.TABLE23_WORKLOADS["ring_512k"]
+    th, p = w.state()
+    ctx = lrmd.Context(RING, w.N, w.eps)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2
+    ctx.set_state(th, p)
+    f = ctx.forces().cpu().numpy()
+    ctx.step(1, w.dt)
+    th1, p1 = ctx.state_numpy()
+    f1 = ctx.forces().cpu().numpy()
+    ctx.close()
+    rows = np.random.default_rng(8).choice(w.N, 2048, replace=False)
+    for state, got in ((th, f), (th1, f1)):
+        r0, _, A0, _ = ref.forces_rows(RING, w.eps, state, None, rows, form=0, with_abs=True)
+        _check_forces(RING, (got[rows], None), (r0, None), (A0, None))
+    assert abs(math.fsum(p1) - math.fsum(p)) <= 1e-12 * math.fsum(np.abs(p))
