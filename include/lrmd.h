@@ -80,8 +80,9 @@ enum {
                                     in one cooperative launch, a grid barrier per substage; falls back to 0 if the device
                                     refuses the cooperative launch); -1 = choose from N (3 up to 20,480, 4 up to 1,070,336,
                                     1 beyond; shards: 0 below 1e6, else 1)                                                  */
-    LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape (threads, i per thread, CTAs per SM, unroll)
-                                    of the pair kernels (-1 = choose)                                          */
+    LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape of the pair kernels (-1 = choose).  Ordered kernels:
+                                    0 = 128 threads x 4 rows, 1 = 128 x 8, 2 = 256 x 4.  Symmetric and band kernels:
+                                    0 = 4 rows per lane, 1 (and 2) = 8; fp32 band kernel: 2 = 16 rows per lane            */
     LRMD_OPT_PAIR_SLOTS = 7,     /* read-only (lrmd_get_option): partial force rows per particle          */
     LRMD_OPT_PAIR_SYMMETRIC = 8, /* pair models: force kernels that evaluate every UNORDERED pair once and add +f / -f to
                                     both particles (the paper declines this): 1 = warp-level
