@@ -238,3 +238,23 @@ def test_ring_512k_paper_table2_size_sampled_rows(lrmd, ref, torch, inputs):
         r0, _, A0, _ = ref.forces_rows(RING, w.eps, state, None, rows, form=0, with_abs=True)
         _check_forces(RING, (got[rows], None), (r0, None), (A0, None))
     assert abs(math.fsum(p1) - math.fsum(p)) <= 1e-12 * math.fsum(np.abs(p))
+
+
+def test_band_kernel_beyond_the_l2_capped_height(lrmd, ref, torch):
+    """N = 3,000,001 (ragged; 2.9x config 5): the scratch rows of the L2-resident band height would pass 1 GiB, so the
+    unconstrained height is used (about 1.4 GB of scratch); one launch per force evaluation; forces on sampled rows,
+    each against all N, against the oracle."""
+    N = 3_000_001
+    st = _state(GRAV2D, N, 31)
+    ctx = lrmd.Context(GRAV2D, N, 1e-3)
+    assert ctx.get_option(lrmd.OPT_PAIR_SYMMETRIC) == 2 and ctx.get_option(lrmd.OPT_PAIR_BAND_HEIGHT) > 16
+    assert ctx.workspace_bytes() < 2_000_000_000
+    ctx.set_state(*st)
+    l0 = ctx.launch_count()
+    f = ctx.forces()
+    assert ctx.launch_count() - l0 == 4          # pack, band kernel, fold, copy-out
+    got = tuple(t.cpu().numpy() for t in f)
+    ctx.close()
+    rows = np.unique(np.concatenate([np.arange(0, 64), np.arange(N - 64, N), np.random.default_rng(9).choice(N, 512, replace=False)]))
+    r0, r1, A0, A1 = ref.forces_rows(GRAV2D, 1e-3, st[0], st[1], rows, form=0, with_abs=True)
+    _check_forces(GRAV2D, tuple(g[rows] for g in got), (r0, r1), (A0, A1))
