@@ -66,8 +66,9 @@ enum {
                                     eps >= 1e-30; HMF: LRMD_EUNSUPPORTED                                            */
     LRMD_OPT_PAIR_CTAS = 1,      /* pair models: number of CTAs G the flattened (i-tile, j) space is divided
                                     into, equal shares (0 = choose from N: 148 x resident CTAs x waves)  */
-    LRMD_OPT_GRAPH = 2,          /* 1 = lrmd_step replays a captured CUDA graph of one step (default
-                                    for small N), 0 = plain launches, -1 = choose from N              */
+    LRMD_OPT_GRAPH = 2,          /* HMF substage kernels: 1 = lrmd_step replays a captured CUDA graph of 8 steps
+                                    (24 kernel nodes) for the steady-state steps, 0 = plain launches, -1 = choose (1;
+                                    never for shards, the resident kernels, or while kernel timing is on)          */
     LRMD_OPT_HMF_GRID = 3,       /* HMF: number of CTAs of the fused substage kernel (0 = choose)      */
     LRMD_OPT_KERNEL_TIMING = 4,  /* 1 = bracket every launch of the model's dominant kernel (HMF: the fused
                                     substage kernel; RING/GRAV2D: the pair-force kernel) with a CUDA event

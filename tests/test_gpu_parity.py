@@ -531,7 +531,7 @@ def test_hmf_default_path_switch(lrmd, ref, torch, N):
     st = _state(HMF, N, 1_000 + N % 7)
     ctx = lrmd.Context(HMF, N, 0.0)
     assert ctx.get_option(lrmd.OPT_HMF_VARIANT) == (1 if N > 1_070_336 else 4)
-    assert ctx.get_option(lrmd.OPT_GRAPH) == 0
+    assert ctx.get_option(lrmd.OPT_GRAPH) == (1 if N > 1_070_336 else 0)      # substage kernels: graph replay of 8 steps
     ctx.set_state(*st)
     f = ctx.forces().cpu().numpy()
     f0, _, S0, _ = ref.forces_abs(HMF, 0.0, st[0], None, form=0)
