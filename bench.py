@@ -292,6 +292,16 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                     "peak_source": "derived: 148 SM x 16 SFU lanes x sm_max_mhz (DESIGN.md); FP32 pipe second: %d FADD/FMUL/FFMA per pair"
                                    % (12 if w.model == 1 else 6),
                     "algorithmic_mufu_per_launch": mufu}
+            if w.model == 1:
+                # Ring, half-angle form: 12 FADD/FMUL/FFMA per pair bind before the one MUFU.RSQ (128 FP32 lanes per SM per
+                # clock: 12 / 128 clock per pair against 1 / 16 for the SFU)
+                fp32 = 12.0 * float(w.N) * float(w.N)
+                peak32 = SM_COUNT * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12
+                roof.update({"achieved": fp32 / avg_s / 1e12, "peak": peak32, "unit": "T FP32 instr/s (thread level)",
+                             "frac": fp32 / avg_s / 1e12 / peak32,
+                             "peak_source": "derived: 148 SM x 128 FP32 lanes x sm_max_mhz (DESIGN.md); SFU second: one MUFU.RSQ per pair",
+                             "algorithmic_fp32_instr_per_launch": fp32,
+                             "mufu_frac": mufu / avg_s / 1e12 / peak})
             if symk:
                 roof["note"] = ("symmetric fp32 kernel: one MUFU.RCP and 8 FADD/FFMA per UNORDERED pair (N^2/2 evaluations deliver "
                                 "N^2 pair interactions), ~10.5 issued instructions per evaluation: instruction issue binds before "
