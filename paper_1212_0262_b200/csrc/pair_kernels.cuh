@@ -1018,14 +1018,19 @@ grav_force_sym_f32_kernel(const float2* __restrict__ js32, SymPart S, float eps,
 // adds the workers in index order.
 template <int MODEL, int R, bool MASK>
 __device__ __forceinline__ void sym_energy_chunk(const double (&a)[R], const double (&b)[R], const long long (&irow)[R],
-                                                 double2 q, long long jq, bool diag, double eps, double onepe,
-                                                 double (&acc)[R], double (&prod)[R], int (&esum)[R]) {
-    const unsigned lane = threadIdx.x & 31u, src = (lane + 31u) & 31u;
+                                                 const double2* __restrict__ spos, long long jbase, long long N, bool diag,
+                                                 double eps, double onepe, double (&acc)[R], double (&prod)[R],
+                                                 int (&esum)[R]) {
+    // spos: the chunk's 32 positions in shared memory (the packet no longer travels by shuffles: a SHFL costs an FP64
+    // issue slot, an LDS none, profiles/r02_fp64_peak.md); lane l meets slot (l + s) mod 32 in step s.
+    const int lane = threadIdx.x & 31;
+    double2 qn = spos[lane];
 #pragma unroll 4
     for (int s = 0; s < 32; ++s) {
-        const double qnx = __shfl_sync(0xffffffffu, q.x, src);
-        const double qny = __shfl_sync(0xffffffffu, q.y, src);
-        const long long jqn = MASK ? __shfl_sync(0xffffffffu, jq, src) : 0;
+        const int idx = (lane + s) & 31;
+        const double2 q = qn;
+        qn = spos[(idx + 1) & 31];
+        const long long jq = MASK ? ((jbase + idx < N) ? jbase + idx : -1) : 0;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             // counted: both particles exist, and inside the tile's own chunks only j > i
@@ -1048,15 +1053,14 @@ __device__ __forceinline__ void sym_energy_chunk(const double (&a)[R], const dou
                 prod[r] = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(prod[r]));
             }
         }
-        q.x = qnx;
-        q.y = qny;
-        if (MASK) jq = jqn;
     }
 }
 
 template <int MODEL, int R>
 __global__ void __launch_bounds__(kSymThreads, 2)
 pair_energy_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, double pre, double* __restrict__ vpart) {
+    __shared__ double2 wpos_all[kSymThreads / 32][32];
+    double2* wpos = wpos_all[threadIdx.x >> 5];
     const int w = blockIdx.x * (kSymThreads / 32) + (threadIdx.x >> 5);
     if (w >= S.G) return;
     const int lane = threadIdx.x & 31;
@@ -1108,8 +1112,11 @@ pair_energy_sym_kernel(const double2* __restrict__ js, SymPart S, double eps, do
         }
         const bool diag = cchunk < (ctile + 1) * R;
         const bool masked = diag || (ragged && (ctile == S.ntiles - 1 || cchunk == S.nchunks - 1));
-        if (masked) sym_energy_chunk<MODEL, R, true>(a, b, irow, q, j < N ? j : -1, diag, eps, onepe, acc, prod, esum);
-        else sym_energy_chunk<MODEL, R, false>(a, b, irow, q, 0, false, eps, onepe, acc, prod, esum);
+        wpos[lane] = q;
+        __syncwarp();
+        if (masked) sym_energy_chunk<MODEL, R, true>(a, b, irow, wpos, (long long)cchunk * 32, N, diag, eps, onepe, acc, prod, esum);
+        else sym_energy_chunk<MODEL, R, false>(a, b, irow, wpos, 0, N, false, eps, onepe, acc, prod, esum);
+        __syncwarp();      // every lane has read the buffer before the next unit overwrites it
         if (tile_done || !more) {
             close_tile();
             if (more) load_tile(tile);
