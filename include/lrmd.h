@@ -54,7 +54,8 @@ enum {
     LRMD_ESTATE = -2,        /* state or workspace not set                                     */
     LRMD_ECUDA = -3,         /* a CUDA call failed; see lrmd_last_cuda_error                   */
     LRMD_EUNSUPPORTED = -4,  /* valid request this build does not implement                    */
-    LRMD_ECOLL = -5          /* a collective callback of a sharded context returned non-zero   */
+    LRMD_ECOLL = -5,         /* a collective callback of a sharded context returned non-zero   */
+    LRMD_ETOOBIG = -6        /* lrmd_hmf_forces_static: N exceeds LRMD_STATIC_MAX_N (the built-in scratch array) */
 };
 
 /* lrmd_set_option keys */
@@ -179,6 +180,41 @@ typedef int (*lrmd_allgather_fn)(void* device_all, int64_t elem_bytes, int64_t i
                                  void* cuda_stream, void* user);
 int lrmd_set_shard(lrmd_ctx* ctx, int64_t N_total, int64_t i0, lrmd_allreduce_fn allreduce, lrmd_allgather_fn allgather,
                    void* user);
+
+/* HMF force for callers that have no way to provide scratch memory.
+ *
+ * Every other call above needs a workspace that the caller allocates (lrmd_workspace_bytes -> cudaMalloc or a torch
+ * tensor -> lrmd_set_workspace).  Some callers cannot do that: a plug-in whose host application grabbed all of the
+ * device memory for its own pool at start-up and hands the plug-in nothing but input and output pointers; a routine
+ * called from inside a latency-critical loop, where cudaMalloc / cudaFree are off limits because they stall the whole
+ * device; a C interface that was fixed before a workspace argument could be added.  This one call serves them.  It
+ * computes, for N particles of the HMF model,
+ *     f_i = cos(theta_i) My - sin(theta_i) Mx,  (Mx, My) = (1/N) sum_j (cos theta_j, sin theta_j)      PAPER.md:73-77 eqs.(6)-(7)
+ * exactly as lrmd_forces does, needs no context and no workspace, and calls no cudaMalloc, cudaFree or any other
+ * allocating routine — neither on the first call nor later.  Its scratch, one (sum cos, sum sin) pair per CTA of the
+ * reduction kernel, lives in an array built into the library: LRMD_STATIC_SCRATCH_BYTES (64 KiB) of device memory,
+ * held on every GPU that loads liblrmd.so until the process exits, whether or not this call is ever used.
+ *
+ *   theta_device  DEVICE, N doubles, 8-byte aligned, read only            f_device  DEVICE, N doubles, written
+ *   N             1 .. LRMD_STATIC_MAX_N (4,194,304 = 4096 CTA sums x 1024 particles each).  A larger N does not fit
+ *                 the built-in array and is refused with LRMD_ETOOBIG before anything is launched; use a context.
+ *   cuda_stream   the two kernels (per-CTA sums, then the forces) are enqueued on it; the call does not synchronise
+ *   cuda_error_host  HOST, may be NULL: receives the cudaError_t (as int) behind an LRMD_ECUDA return, else 0
+ *
+ * The current device must be the one that owns theta_device, f_device and the stream.
+ * First call on a device: the library looks up the device address of its scratch array once per device
+ * (cudaGetSymbolAddress; the array's name is not a usable pointer in host code) and remembers it; this lookup is
+ * thread-safe.  Make that first call on each device before starting any stream capture.
+ * All calls on a device share the one array and it keeps whatever the previous call left there.  Nothing in it has to
+ * start at zero: each call overwrites every entry it later reads.  Calls issued to the SAME stream are ordered and
+ * safe.  Calls that can run at the same time on one GPU (different streams, different host threads, different
+ * processes each have their own copy — only calls within one process share it) overwrite each other's sums and
+ * return wrong forces: serialise them yourself.
+ * Other returns: LRMD_EINVAL (NULL or misaligned pointer, N < 1), LRMD_EUNSUPPORTED (device ordinal >= 64). */
+#define LRMD_STATIC_MAX_N 4194304
+#define LRMD_STATIC_SCRATCH_BYTES 65536
+int lrmd_hmf_forces_static(const double* theta_device, double* f_device, int64_t N, void* cuda_stream,
+                           int* cuda_error_host);
 
 /* Set an option (keys above).  Unknown key or bad value: LRMD_EINVAL. */
 int lrmd_set_option(lrmd_ctx* ctx, int key, int64_t value);

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <tuple>
 #include <utility>
@@ -998,6 +999,74 @@ bool finite_pos(double x) { return std::isfinite(x) && x > 0.0; }
 
 }  // namespace
 
+// ---- lrmd_hmf_forces_static: the one call whose scratch is built into the library --------------------
+// For callers that cannot hand over a workspace (see include/lrmd.h).  The per-CTA (sum cos, sum sin) pairs of the
+// reduction go to the file-scope array below instead of the caller's workspace: 4096 pairs = 64 KiB, resident on every
+// GPU that loads the library.  One CTA sums a fixed block of 1024 particles, so the number of CTAs — and with it the
+// scratch — grows with N; 4096 CTAs cover LRMD_STATIC_MAX_N particles and a larger N is refused.
+constexpr int kStaticMaxCtas = 4096;
+constexpr int kStaticPerThread = 4;
+constexpr int kStaticPerCta = kStaticPerThread * lrmd::kHmfThreads;   // 1024
+constexpr int kStaticMaxDevices = 64;
+static_assert((long long)kStaticMaxCtas * kStaticPerCta == LRMD_STATIC_MAX_N, "lrmd.h states this limit");
+static_assert(sizeof(double2) * kStaticMaxCtas == LRMD_STATIC_SCRATCH_BYTES, "lrmd.h states this size");
+
+static __device__ __align__(256) double2 g_lrmd_static_partials[kStaticMaxCtas];
+
+// Variant of the reduce-only substage kernel (hmf_substage_kernel<false, false, false, true>): same per-particle
+// arithmetic and the same fixed block-sum tree, but CTA b always owns particles [1024 b, 1024 b + 1024) (no grid
+// stride, scalar loads: theta needs 8-byte alignment only) and writes its pair to partial_out[b], which the host passes
+// as the device address of g_lrmd_static_partials.  Every entry the force kernel reads afterwards (0 .. gridDim.x - 1)
+// is written here first, so the array never needs clearing.
+__global__ void __launch_bounds__(lrmd::kHmfThreads)
+hmf_reduce_static_kernel(const double* __restrict__ theta, long long N, double2* __restrict__ partial_out) {
+    __shared__ double scratch[2 * (lrmd::kHmfThreads / 32)];
+    const long long base = (long long)blockIdx.x * kStaticPerCta + threadIdx.x;
+    double r[2] = {0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < kStaticPerThread; ++k) {
+        const long long i = base + (long long)k * lrmd::kHmfThreads;
+        if (i < N) {
+            double s, c;
+            lrmd::sincos_any(theta[i], s, c);
+            r[0] += c;
+            r[1] += s;
+        }
+    }
+    lrmd::block_sum<lrmd::kHmfThreads, 2>(r, scratch);
+    if (threadIdx.x == 0) partial_out[blockIdx.x] = make_double2(r[0], r[1]);
+}
+
+namespace {
+
+// Device address of g_lrmd_static_partials on the current device.  In host code the array's name stands for a host-side
+// shadow object, not for device memory, so the address is asked for once per device (with that device current) and
+// kept.  cudaGetSymbolAddress allocates nothing: the array is part of the loaded module.
+std::mutex g_static_mutex;
+double2* g_static_addr[kStaticMaxDevices] = {};
+
+int static_partials(double2** out, cudaError_t* err) {
+    int dev = -1;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) { (void)cudaGetLastError(); return LRMD_ECUDA; }
+    if (dev < 0 || dev >= kStaticMaxDevices) return LRMD_EUNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        *err = cudaGetSymbolAddress(&p, g_lrmd_static_partials);
+        if (*err != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            if (*err == cudaSuccess) *err = cudaErrorInvalidSymbol;
+            return LRMD_ECUDA;
+        }
+        g_static_addr[dev] = static_cast<double2*>(p);
+    }
+    *out = g_static_addr[dev];
+    return LRMD_OK;
+}
+
+}  // namespace
+
 // =========================================== C ABI =====================================================
 
 extern "C" {
@@ -1218,6 +1287,45 @@ int lrmd_energy(lrmd_ctx* c, double* out4_device, void* cuda_stream) {
     return L.rc;
 }
 
+int lrmd_hmf_forces_static(const double* theta_device, double* f_device, int64_t N, void* cuda_stream,
+                           int* cuda_error_host) {
+    // no context, no workspace, no allocation: the per-CTA sums go to g_lrmd_static_partials (see above and lrmd.h)
+    if (cuda_error_host) *cuda_error_host = 0;
+    if (!theta_device || !f_device || N < 1) return LRMD_EINVAL;
+    if (((uintptr_t)theta_device % 8) != 0 || ((uintptr_t)f_device % 8) != 0) return LRMD_EINVAL;
+    if (N > (int64_t)LRMD_STATIC_MAX_N) return LRMD_ETOOBIG;     // would need more CTA sums than the array holds
+    cudaError_t e = cudaSuccess;
+    double2* partials = nullptr;
+    const int rc = static_partials(&partials, &e);    // first call on this device: looks the address up
+    if (rc != LRMD_OK) {
+        if (cuda_error_host) *cuda_error_host = (int)e;
+        return rc;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int ctas = (int)((N + kStaticPerCta - 1) / kStaticPerCta);     // <= kStaticMaxCtas
+    long long n = (long long)N;
+    const double2* sums = partials;
+    {
+        void* args[] = {(void*)&theta_device, (void*)&n, (void*)&partials};
+        e = cudaLaunchKernel((const void*)hmf_reduce_static_kernel, dim3((unsigned)ctas), dim3(kHmfThreads), args, 0, stream);
+    }
+    if (e == cudaSuccess) {
+        // the force kernel of lrmd_forces, unchanged: every CTA re-sums the `ctas` pairs in index order
+        int64_t g = (N + kHmfThreads - 1) / kHmfThreads;
+        if (g > kHmfMaxGrid) g = kHmfMaxGrid;
+        double inv_n = 1.0 / (double)N;
+        int g_in = ctas;
+        void* args[] = {(void*)&theta_device, (void*)&f_device, (void*)&n, (void*)&inv_n, (void*)&sums, (void*)&g_in};
+        e = cudaLaunchKernel((const void*)hmf_force_kernel, dim3((unsigned)g), dim3(kHmfThreads), args, 0, stream);
+    }
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (cuda_error_host) *cuda_error_host = (int)e;
+        return LRMD_ECUDA;
+    }
+    return LRMD_OK;
+}
+
 int lrmd_set_shard(lrmd_ctx* c, int64_t N_total, int64_t i0, lrmd_allreduce_fn allreduce, lrmd_allgather_fn allgather,
                    void* user) {
     if (!c) return LRMD_EINVAL;
@@ -1391,6 +1499,7 @@ const char* lrmd_strerror(int code) {
         case LRMD_ECUDA: return "CUDA error (see lrmd_last_cuda_error)";
         case LRMD_EUNSUPPORTED: return "not implemented in this build";
         case LRMD_ECOLL: return "a collective callback of a sharded context failed";
+        case LRMD_ETOOBIG: return "N exceeds LRMD_STATIC_MAX_N: the library's built-in scratch array is too small, use a context";
         default: return "unknown error code";
     }
 }

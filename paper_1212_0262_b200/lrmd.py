@@ -16,7 +16,8 @@ import ctypes as C
 import os
 
 HMF, RING, GRAV2D = 0, 1, 2
-OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED, ECOLL = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ESTATE, ECUDA, EUNSUPPORTED, ECOLL, ETOOBIG = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_N = 4194304      # LRMD_STATIC_MAX_N of include/lrmd.h
 OPT_PAIR_PRECISION, OPT_PAIR_CTAS, OPT_GRAPH, OPT_HMF_GRID, OPT_KERNEL_TIMING = 0, 1, 2, 3, 4
 OPT_HMF_VARIANT, OPT_PAIR_VARIANT, OPT_PAIR_SLOTS, OPT_PAIR_SYMMETRIC, OPT_PAIR_SYM_TILES = 5, 6, 7, 8, 9
 OPT_PAIR_FUSE_UPDATE = 10
@@ -29,7 +30,7 @@ SYMBOLS = (
     "lrmd_step", "lrmd_step_host", "lrmd_forces", "lrmd_energy", "lrmd_set_option", "lrmd_get_option",
     "lrmd_launch_count", "lrmd_kernel_time", "lrmd_last_cuda_error", "lrmd_strerror", "lrmd_coefficients", "lrmd_host_sincos",
     "lrmd_pair_partition", "lrmd_step_observe", "lrmd_set_shard", "lrmd_pair_sym_partition", "lrmd_fp64_peak",
-    "lrmd_pair_band_partition",
+    "lrmd_pair_band_partition", "lrmd_hmf_forces_static",
 )
 
 _lib = None
@@ -85,6 +86,7 @@ def load(build_if_missing: bool = True):
     lib.lrmd_pair_sym_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
     lib.lrmd_pair_band_partition.argtypes = [_vp, _i64, _vp, C.POINTER(_i64)]
     lib.lrmd_fp64_peak.argtypes = [_int, _int, _int, _int, _int, _vp, C.c_size_t, C.POINTER(_dbl), _vp]
+    lib.lrmd_hmf_forces_static.argtypes = [_vp, _vp, _i64, _vp, C.POINTER(_int)]
     for name in SYMBOLS:
         if name != "lrmd_strerror":
             getattr(lib, name).restype = _int
@@ -138,6 +140,17 @@ def lrmd_forces(ctx, f0: int, f1: int | None = None, stream: int = 0):
 
 def lrmd_energy(ctx, out4_device: int, stream: int = 0):
     return load().lrmd_energy(ctx, out4_device, stream)
+
+
+def lrmd_hmf_forces_static(theta_device: int, f_device: int, N: int, stream: int = 0):
+    """HMF forces without a context or a workspace, for callers that cannot allocate scratch (a plug-in inside an
+    application that owns all device memory, a loop where cudaMalloc's device-wide stall is not acceptable): the
+    library's built-in 64 KiB array holds the per-CTA sums, so N <= STATIC_MAX_N (else ETOOBIG).  Raw device pointers
+    as ints.  Returns (rc, cudaError).  All calls share that one array: calls on one stream are safe, calls that may
+    overlap on the GPU are not.  Make the first call on each device outside any stream capture.  See include/lrmd.h."""
+    err = _int(0)
+    rc = load().lrmd_hmf_forces_static(theta_device, f_device, int(N), stream, C.byref(err))
+    return rc, int(err.value)
 
 
 def lrmd_set_option(ctx, key: int, value: int):
