@@ -7,10 +7,11 @@
 A bench "step" is one complete integrator time step of the workload (three force
 evaluations + the kick/drift updates — what the paper's Tables 1-3 time).  The primary workload is
 BASELINE.json configs[4], the largest single-GPU configuration (2D self-gravitating, N = 1,048,576,
-eps = 1e-3, dt = 0.005, fp64); with one GPU and without --only the other configs are measured too and
-reported under "others" in the same line, together with the ordered-pair kernels (the paper's own
-scheme, LRMD_OPT_PAIR_SYMMETRIC = 0) on the pair configs, config 5's fp32-pair variant and the HMF
-sizes of the paper's Table 1.
+eps = 1e-3, dt = 0.005, fp64).  The LAST stdout line is that headline alone, trimmed to under 4 KB (the
+driver keeps only the tail of stdout).  With one GPU and without --only / --no-others the other configs are
+measured too, together with the ordered-pair kernels (the paper's own scheme, LRMD_OPT_PAIR_SYMMETRIC = 0)
+on the pair configs, config 5's fp32-pair variant and the sizes of the paper's Tables 1-3: their full
+objects go to gpurun_out/bench_others.json (with the untrimmed headline) and one short line each to stderr.
 
 Numbers reported (all measured in this process, never under a profiler):
   value      whole-job throughput, state resident in HBM, CUDA events on the launching stream
@@ -18,10 +19,11 @@ Numbers reported (all measured in this process, never under a profiler):
              evaluations + D2H inside the timed region
   roofline   the dominant kernel (pair-force kernel / HMF fused substage): work per force evaluation (pair
              models) or per launch (HMF) / its device time from event pairs around every launch (second pass).
-             Pair models: EXECUTED flops against 148 x 64 x 2 x f_max; the symmetric kernel evaluates every
-             unordered pair once, so its executed work per delivered pair is about half the ordered kernels'
-             (roofline.note gives the ordered-pair-convention figure as well).  HMF: 32 B per particle-substage
-             against the measured HBM copy bandwidth.
+             Pair models (fp64): `frac` = EXECUTED FP64 instructions / s over 148 x 64 x f_max (the
+             acceptance number), `flop_frac` = executed flops (FMA = 2) over 148 x 64 x 2 x f_max beside it; the
+             symmetric kernels evaluate every unordered pair once, so their executed work per delivered pair is about
+             half the ordered kernels' (`flop_frac_ordered_convention` gives that reading).  HMF: 32 B per
+             particle-substage against the measured HBM copy bandwidth.
   energy     lrmd_energy timed apart from the steps
   cpu_baseline  the oracle (oracle/lrmd_ref.cpp), as it stands, on this box's host cores, bounded sample
 
@@ -59,7 +61,7 @@ HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel come from the committed
 # `ncu --set full` captures: profiles/r02_traffic.csv names, per bench entry, the kernel, the two byte counts and
-# the capture they were read from (profiles/r02_summary.md gives the commands).
+# the capture they were read from (profiles/r02_ncu_full.md gives the commands).
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
 
 
@@ -171,7 +173,7 @@ def units_per_force(w):
 
 
 def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs=False, ordered_pairs=False,
-                 force_symmetric=False, roofline_steps=2000, e2e_steps=20, fp64_peak=None):
+                 force_symmetric=False, roofline_steps=2000, e2e_steps=20, fp64_peak=None, with_energy=True):
     import torch
     from paper_1212_0262_b200 import lrmd
 
@@ -220,6 +222,12 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
 
     # warm-up (also caches the force at the current positions)
     timed_pass(W)
+    if resident_by_design and ctx.get_option(lrmd.OPT_HMF_VARIANT) not in (3, 4):
+        # the device refused the cooperative launch and the library fell back to the streaming kernels: flush after all
+        resident_by_design = False
+        if not larger_than_l2:
+            flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+        timed_pass(W)
     barrier()
     sampler = ClockSampler(torch.cuda.current_device()).start()
     l0 = ctx.launch_count()
@@ -240,7 +248,7 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
     out = {
         "metric": metric, "value": value, "unit": unit, "ms_per_step": ms_max / K,
         "gpu_launches": int(launches), "clocks": clocks,
-        "l2": l2_statement(w),
+        "l2": l2_statement(w, hmf_resident=resident_by_design),
         "options": {"pair_ctas": ctx.get_option(lrmd.OPT_PAIR_CTAS), "pair_variant": ctx.get_option(lrmd.OPT_PAIR_VARIANT),
                     "pair_slots": ctx.get_option(lrmd.OPT_PAIR_SLOTS), "graph": ctx.get_option(lrmd.OPT_GRAPH),
                     "hmf_grid": ctx.get_option(lrmd.OPT_HMF_GRID), "hmf_variant": ctx.get_option(lrmd.OPT_HMF_VARIANT),
@@ -309,26 +317,27 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
                                 % (float(w.N) * float(w.N) / avg_s / 1e12 / peak))
         else:
             kernel = {0: "pair_force_kernel", 1: "pair_force_sym_kernel", 2: "pair_force_band_kernel"}[symk]
+            # (i) pipe utilisation = EXECUTED FP64 instructions / s over 148 x 64 x f_max — the acceptance
+            # number, reported as `frac`; (ii) the flop fraction (FMA = 2) beside it.  The symmetric kernels evaluate every
+            # unordered pair once: their executed work per delivered pair is about half the ordered kernels'.
             flop = (SYM_PAIR_FLOP if symk else PAIR_FLOP)[w.model] * w.N * w.N
-            achieved = flop / avg_s / 1e12
-            peak = SM_COUNT * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-            instr_rate = (SYM_PAIR_FP64_INSTR if symk else PAIR_FP64_INSTR)[w.model] * w.N * w.N / avg_s
-            roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "peak_source": "derived: 148 SM x 64 FP64 lanes x 2 flop x sm_max_mhz (DESIGN.md)",
-                    "algorithmic_flop_per_launch": flop,
-                    "fp64_pipe_frac_at_max_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6),
-                    "fp64_pipe_frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
+            instr = (SYM_PAIR_FP64_INSTR if symk else PAIR_FP64_INSTR)[w.model] * w.N * w.N
+            instr_rate = instr / avg_s
+            peak_instr = SM_COUNT * FP64_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
+            roof = {"bound": "alu", "achieved": instr_rate / 1e12, "peak": peak_instr / 1e12, "unit": "T FP64 instr/s",
+                    "frac": instr_rate / peak_instr,
+                    "peak_source": "derived: 148 SM x 64 FP64 lanes x sm_max_mhz (DESIGN.md 6)",
+                    "algorithmic_fp64_instr_per_launch": instr,
+                    "tflops": flop / avg_s / 1e12, "peak_tflops": 2.0 * peak_instr / 1e12,
+                    "flop_frac": flop / avg_s / (2.0 * peak_instr),
+                    "frac_at_held_clock": instr_rate / (SM_COUNT * FP64_LANES_PER_SM * clk * 1e6)}
             if fp64_peak is not None:
                 # the committed microbenchmark (lrmd_fp64_peak): what the FP64 pipe sustains on this box
-                roof["peak_measured"] = fp64_peak["dfma_tflops"]
-                roof["frac_of_peak_measured"] = achieved / fp64_peak["dfma_tflops"]
-                roof["peak_measured_what"] = fp64_peak["what"]
-                roof["fp64_pipe_frac_of_measured_issue_rate"] = instr_rate / fp64_peak["dmul_instr_per_s"]
+                roof["frac_of_measured_issue_rate"] = instr_rate / fp64_peak["dmul_instr_per_s"]
+                roof["flop_frac_of_measured_dfma"] = flop / avg_s / 1e12 / fp64_peak["dfma_tflops"]
             if symk:
-                roof["note"] = ("symmetric kernel: every unordered pair evaluated once (N^2/2 evaluations deliver N^2 pair "
-                                "interactions); flops and instructions are the EXECUTED ones; by the ordered-pair convention "
-                                "(%g flop per delivered pair) the same launch reads %.3f of peak"
-                                % (PAIR_FLOP[w.model], PAIR_FLOP[w.model] * w.N * w.N / avg_s / 1e12 / peak))
+                # by the ordered-pair convention (16 / 18 flop per delivered pair) the same launch would read:
+                roof["flop_frac_ordered_convention"] = PAIR_FLOP[w.model] * w.N * w.N / avg_s / (2.0 * peak_instr)
         entry = w.key + ("_f32pairs" if f32_pairs else "") + ("_ordered_pairs" if (w.model != 0 and not symk) else "")
         traffic, tsrc = ncu_traffic(entry, kernel)
         if w.model == 0:
@@ -348,11 +357,11 @@ def run_workload(w, K, W, dist_ctx, with_e2e=True, with_roofline=True, f32_pairs
         out["roofline"] = roof
 
     # ---- energy sums (rows a-E1..a-E3), timed apart from the steps
-    if w.key != "grav2d_1m":
+    if with_energy:
         ctx.energy()
         torch.cuda.synchronize(dev)
         ts = []
-        for _ in range(5):
+        for _ in range(2 if w.N >= 500_000 and w.model != 0 else 5):    # config 5: about half a second per O(N^2) sweep
             if flush is not None:
                 flush.fill_(1)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -431,24 +440,31 @@ def oracle_sample_rate(w, seconds, nthreads=0):
     return R * w.N / el, f"forces on {R} sampled rows x all {w.N} j ({what}), OpenMP over rows", threads
 
 
-def l2_statement(w):
-    """How the timed iterations keep L2 from flattering the number (the same for every arm of a workload)."""
+HMF_RESIDENT_MAX_N = 1_070_336      # up to here the default HMF kernel keeps the state on chip (lrmd.h, LRMD_OPT_HMF_VARIANT)
+
+
+def l2_statement(w, hmf_resident=None):
+    """How the timed iterations keep L2 from flattering the number.  Decided by the SAME two predicates that switch the
+    flush in run_workload: the state is larger than L2, or the HMF kernel in use keeps the state on chip for the whole call
+    (`hmf_resident`; None = what the library chooses by default for this N, which is all the reference arm can know)."""
     narr = 4 if w.model == 2 else 2
     state_bytes = narr * w.N * 8
+    if hmf_resident is None:
+        hmf_resident = w.model == 0 and w.N <= HMF_RESIDENT_MAX_N
     if state_bytes > L2_BYTES:
         return "inputs larger than L2 (%.0f MB state)" % (state_bytes / 1e6)
-    if w.model == 0 and w.N < 1_000_000:
-        return ("not flushed: the %.2f MB state stays on chip (registers of one cluster / shared memory of the grid) for all "
-                "steps of the one launch, by design; latency-bound case" % (state_bytes / 1e6))
+    if hmf_resident:
+        return "not flushed: %.2f MB state kept on chip by the resident kernel for all steps of one launch" % (state_bytes / 1e6)
     return "L2 flushed (256 MiB write) before every timed step"
 
 
-def workload_config(w, world):
-    """The `config` object of the JSON line: the workload, identical for the b200 and the reference arm."""
+def workload_config(w, world, l2=None):
+    """The `config` object of the JSON line: the workload, identical for the b200 and the reference arm (`l2` = the
+    statement of the run that was timed; None = the default choice for this N)."""
     return {"workload": w.key, "model": ["hmf", "ring", "grav2d"][w.model], "N": w.N, "eps": w.eps, "dt": w.dt,
             "step": "one 4th-order time step = 3 force evaluations + kick/drift updates (PAPER.md:54-63)",
             "parallelism": "replicas only (no sharding, no collectives)" if world > 1 else "1 GPU",
-            "l2": l2_statement(w)}
+            "l2": l2 or l2_statement(w)}
 
 
 def run_reference(args, w):
@@ -597,6 +613,127 @@ def fp64_peak_summary():
                        dfma["sm_mhz"])}
 
 
+# ---- the one stdout line --------------------------------------------------------------------------------------
+# The driver keeps only the tail of stdout, so the LAST line must be small: the headline object alone, trimmed to the keys
+# below and bounded by HEADLINE_MAX_BYTES.  Everything else (the other configs, the paper's table sizes, the ordered-pair
+# and fp32 variants, the long explanations) goes to OTHERS_FILE and, one compact line per entry, to stderr.  What the
+# roofline keys mean is written once, instead of in every line.
+HEADLINE_MAX_BYTES = 4000
+OTHERS_FILE = os.path.join("gpurun_out", "bench_others.json")
+
+HEADLINE_KEYS = ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                 "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "energy",
+                 "options", "others_file")
+ROOFLINE_KEYS = ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel", "kernel_avg_ms", "kernel_share_of_step",
+                 "peak_source", "flop_frac", "tflops", "peak_tflops", "frac_at_held_clock", "frac_of_measured_issue_rate",
+                 "flop_frac_of_measured_dfma", "flop_frac_ordered_convention", "mufu_frac", "traffic_ratio", "traffic_source",
+                 "workspace_bytes")
+SUB_KEYS = {
+    "config": ("workload", "model", "N", "eps", "dt", "parallelism", "l2"),
+    "clocks": ("sm_mhz", "sm_max_mhz", "reasons", "samples"),
+    "e2e": ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "steps_per_call"),
+    "roofline": ROOFLINE_KEYS,
+    "cpu_baseline": ("value", "unit", "cores", "kind", "sample"),
+    "energy": ("ms_per_call", "pair_interactions_per_s"),
+}
+
+
+def _short(v, limit=160):
+    if isinstance(v, float):
+        return float("%.6g" % v)
+    if isinstance(v, str) and len(v) > limit:
+        return v[: limit - 3] + "..."
+    return v
+
+
+def headline(line: dict) -> dict:
+    """The object printed as the last stdout line: `line` cut down to HEADLINE_KEYS / SUB_KEYS, floats to 6 digits, long
+    strings clipped; if it is still over HEADLINE_MAX_BYTES the optional keys go, last first (never the contract's)."""
+    out = {}
+    for k in HEADLINE_KEYS:
+        if k not in line:
+            continue
+        v = line[k]
+        if isinstance(v, dict) and k in SUB_KEYS:
+            v = {kk: _short(v[kk]) for kk in SUB_KEYS[k] if kk in v and v[kk] is not None or kk == "traffic" and kk in v}
+        elif isinstance(v, dict):
+            v = {kk: _short(vv) for kk, vv in v.items()}
+        else:
+            v = _short(v)
+        out[k] = v
+    optional = [("options", None), ("energy", None)] + [("roofline", kk) for kk in reversed(ROOFLINE_KEYS[6:])]
+    while len(json.dumps(out)) > HEADLINE_MAX_BYTES and optional:
+        k, kk = optional.pop(0)
+        if kk is None:
+            out.pop(k, None)
+        elif isinstance(out.get(k), dict):
+            out[k].pop(kk, None)
+    return out
+
+
+def write_others(others: dict, line: dict):
+    """Side file with the full objects (headline untrimmed + the other entries); returns its path or None."""
+    try:
+        os.makedirs(os.path.dirname(os.path.join(ROOT, OTHERS_FILE)), exist_ok=True)
+        with open(os.path.join(ROOT, OTHERS_FILE), "w") as fh:
+            json.dump({"headline": line, "others": others}, fh, indent=1)
+        return OTHERS_FILE
+    except OSError:
+        return None
+
+
+def run_others(w, inputs, peak):
+    """The entries beside the headline (1 GPU, default run): the other BASELINE.json configs, the paper's Table 1-3 sizes,
+    the ordered-pair kernels (the paper's own scheme) and the fp32-pair variants.  An entry that fails is recorded, not
+    raised: the headline line must still be printed."""
+    keep = ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options", "clocks", "roofline", "e2e", "energy")
+    others = {}
+
+    def add(name, ow, steps, **kw):
+        try:
+            r = run_workload(ow, steps, 3, None, fp64_peak=peak, **kw)
+            others[name] = {k: r[k] for k in keep if k in r}
+            others[name]["steps"] = steps
+            roof = r.get("roofline") or {}
+            print(json.dumps({"other": name, "value": _short(r["value"]), "unit": r["unit"], "ms_per_step": _short(r["ms_per_step"]),
+                              "kernel": roof.get("kernel"), "frac": _short(roof.get("frac"))}), file=sys.stderr)
+        except Exception as exc:      # noqa: BLE001 — recorded in the side file
+            others[name] = {"error": "%s: %s" % (type(exc).__name__, exc)}
+            print(json.dumps({"other": name, "error": others[name]["error"]}), file=sys.stderr)
+
+    for key in ("ring_16k", "grav2d_64k", "hmf_5e7", "grav2d_1m", "hmf_1e4"):
+        if key == w.key:
+            continue
+        add(key, inputs.WORKLOADS[key], DEFAULT_STEPS[key], with_e2e=(key != "grav2d_1m"), roofline_steps=(3 if key == "grav2d_1m" else 2000))
+    # HMF at the sizes of the paper's Table 1 (PAPER.md:142-146) that lie between configs 1 and 4
+    for key, ow in inputs.TABLE1_WORKLOADS.items():
+        if key != w.key:
+            add(key, ow, DEFAULT_STEPS[key], with_e2e=False)
+    # pair-model sizes of the paper's Tables 2 and 3 beyond the configs (PAPER.md:150-166)
+    for key, ow in inputs.TABLE23_WORKLOADS.items():
+        if key != w.key:
+            add(key, ow, DEFAULT_STEPS[key], with_e2e=False, roofline_steps=3)
+    for key, sec in inputs.PAPER_SECONDS_PER_STEP.items():
+        if key in others:
+            others[key]["paper_seconds_per_step_one_gk104"] = sec      # PAPER.md Tables 1-3: context, other hardware
+    # the paper's own scheme, every ORDERED pair (PAPER.md:108), on the configs where a symmetric kernel is the default
+    for key in ("ring_16k", "grav2d_64k", "grav2d_1m"):
+        steps = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]
+        add(key + "_ordered_pairs", inputs.WORKLOADS[key], steps, with_e2e=False, ordered_pairs=True, with_energy=(key != "grav2d_1m"),
+            roofline_steps=3 if key == "grav2d_1m" else 2000)
+    # config 5's optional variant (PAPER.md:110): fp32 pair arithmetic, fp64 accumulation across chunks
+    add("grav2d_1m_f32pairs", inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], with_e2e=False, f32_pairs=True, roofline_steps=3,
+        with_energy=False)
+    add("grav2d_1m_f32pairs_ordered_pairs", inputs.WORKLOADS["grav2d_1m"], 3, with_e2e=False, f32_pairs=True, ordered_pairs=True,
+        roofline_steps=3, with_energy=False)
+    add("ring_16k_f32pairs", inputs.WORKLOADS["ring_16k"], DEFAULT_STEPS["ring_16k"], with_e2e=False, f32_pairs=True)
+    for key, what in (("grav2d_1m_f32pairs", "f32 pair terms, f64 state and accumulation"),
+                      ("ring_16k_f32pairs", "f32 pair terms (half-angle form), f64 state and accumulation")):
+        if "error" not in others.get(key, {"error": 1}):
+            others[key]["dtype"] = what
+    return others
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -604,6 +741,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--workload", default="grav2d_1m")
     ap.add_argument("--only", action="store_true", help="primary workload only (no 'others', no cpu_baseline)")
+    ap.add_argument("--no-others", action="store_true", help="headline with cpu_baseline, without the other entries")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--f32-pairs", action="store_true", help="pair workloads: fp32 pair arithmetic (PAPER.md:110, 136)")
@@ -670,54 +808,22 @@ def main():
         "metric": res["metric"], "value": res["value"], "unit": res["unit"], "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if f32 else "f64", "data": "synthetic",
-        "config": workload_config(w, world), "options": res["options"],
+        "config": workload_config(w, world, l2=res["l2"]), "options": res["options"],
         "clocks": res["clocks"], "e2e": res.get("e2e"), "gpu_launches": res["gpu_launches"],
         "roofline": res.get("roofline"), "energy": res.get("energy"),
     }
 
-    keep = ("metric", "value", "unit", "ms_per_step", "gpu_launches", "l2", "options", "clocks", "roofline", "e2e", "energy")
+    others = None
     if world == 1 and not args.only:
-        others = {}
-
-        def add(name, ow, steps, **kw):
-            r = run_workload(ow, steps, 3, None, fp64_peak=peak, **kw)
-            others[name] = {k: r[k] for k in keep if k in r}
-            others[name]["steps"] = steps
-
-        for key in ("ring_16k", "grav2d_64k", "hmf_5e7", "grav2d_1m", "hmf_1e4"):
-            if key == w.key:
-                continue
-            add(key, inputs.WORKLOADS[key], DEFAULT_STEPS[key], with_e2e=(key != "grav2d_1m"), roofline_steps=(3 if key == "grav2d_1m" else 2000))
-        # HMF at the sizes of the paper's Table 1 that lie between configs 1 and 4
-        for key, ow in inputs.TABLE1_WORKLOADS.items():
-            if key != w.key:
-                add(key, ow, DEFAULT_STEPS[key], with_e2e=False)
-        # pair-model sizes of the paper's Tables 2 and 3 beyond the configs
-        for key, ow in inputs.TABLE23_WORKLOADS.items():
-            if key != w.key:
-                add(key, ow, DEFAULT_STEPS[key], with_e2e=False, roofline_steps=3)
-        for key, sec in inputs.PAPER_SECONDS_PER_STEP.items():
-            if key in others:
-                others[key]["paper_seconds_per_step_one_gk104"] = sec      # PAPER.md Tables 1-3: context, other hardware
-        # the paper's own scheme, every ORDERED pair, on the configs where a symmetric kernel is the default
-        for key in ("ring_16k", "grav2d_64k", "grav2d_1m"):
-            steps = 3 if key == "grav2d_1m" else DEFAULT_STEPS[key]
-            add(key + "_ordered_pairs", inputs.WORKLOADS[key], steps, with_e2e=False, ordered_pairs=True, roofline_steps=3 if key == "grav2d_1m" else 2000)
-        # config 5's optional variant: fp32 pair arithmetic, fp64 accumulation across chunks
-        add("grav2d_1m_f32pairs", inputs.WORKLOADS["grav2d_1m"], DEFAULT_STEPS["grav2d_1m"], with_e2e=False, f32_pairs=True, roofline_steps=3)
-        others["grav2d_1m_f32pairs"]["dtype"] = "f32 pair terms, f64 state and accumulation"
-        add("grav2d_1m_f32pairs_ordered_pairs", inputs.WORKLOADS["grav2d_1m"], 3, with_e2e=False, f32_pairs=True, ordered_pairs=True,
-            roofline_steps=3)
-        add("ring_16k_f32pairs", inputs.WORKLOADS["ring_16k"], DEFAULT_STEPS["ring_16k"], with_e2e=False, f32_pairs=True)
-        others["ring_16k_f32pairs"]["dtype"] = "f32 pair terms (half-angle form), f64 state and accumulation"
-        line["others"] = others
         rate, desc, threads = oracle_sample_rate(w, args.cpu_seconds)
-        line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc,
-                                "note": "the oracle is an unoptimised checker (compensated sums, true division, -O2 without "
-                                        "contraction), not a tuned CPU code: a reported baseline, not a speedup claim"}
+        line["cpu_baseline"] = {"value": rate, "unit": res["unit"], "cores": threads, "kind": "oracle", "sample": desc}
+        if not args.no_others:
+            others = run_others(w, inputs, peak)
 
     if rank == 0:
-        print(json.dumps(line))
+        if others is not None:
+            line["others_file"] = write_others(others, line)
+        print(json.dumps(headline(line)))
     if dist_ctx is not None:
         dist_ctx.barrier()
         dist_ctx.destroy_process_group()
