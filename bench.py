@@ -490,7 +490,7 @@ def run_reference(args, w):
         "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
-    print(json.dumps(line))
+    print(json.dumps(headline(line)))      # trimmed like the b200 arm's line, so that both print the same `config`
     return 0
 
 
