@@ -33,6 +33,17 @@
  *   - Calls on one context are not thread-safe; different contexts are independent.
  *   - Results are bitwise reproducible run to run for fixed (model, N, eps, options): all
  *     reductions use fixed trees and there are no floating-point atomics.
+ *   - Streams: calls on one context must be issued to one stream at a time (or be ordered by the caller's
+ *     events); different contexts may run on different streams concurrently.  No call waits for, or
+ *     enqueues on, any other stream (tests/test_gpu_streams.py).
+ *   - Capturing calls in a CUDA graph: lrmd_step (substage kernels: LRMD_OPT_HMF_VARIANT 0-2; all pair
+ *     kernels), lrmd_forces and lrmd_energy enqueue plain kernel launches only, so the caller may capture them
+ *     on a capturing stream PROVIDED one eager lrmd_step (and one eager call of whatever else is captured) ran
+ *     on the context before: that caches the force and raises the kernels' shared-memory limits, so the
+ *     captured sequence is the steady-state one.  Every replay advances the bound state by the captured
+ *     steps.  The library's own graph replay (LRMD_OPT_GRAPH) stands aside while the stream is capturing.
+ *     Not for capture: lrmd_set_workspace, lrmd_step_host, lrmd_kernel_time (they synchronise) and contexts
+ *     with LRMD_OPT_KERNEL_TIMING on (event records); the resident HMF kernels (variants 3, 4) are untested.
  */
 #ifndef LRMD_H_
 #define LRMD_H_

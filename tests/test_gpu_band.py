@@ -222,7 +222,8 @@ def test_band_fused_potential_at_config3_size(lrmd, ref, torch, inputs):
 def test_ring_512k_paper_table2_size_sampled_rows(lrmd, ref, torch, inputs):
     """The largest Ring run of the paper's Table 2 (N = 512,000) in the default configuration (band
     kernel, I-blocks of 2048 rows): forces on 2,048 sampled rows, each against all N, against the oracle's direct
-    eq.(8) form; K and V after one step against the oracle at the GPU's own state on the same rows' scale."""
+    eq.(8) form, at t = 0 and at the GPU's own angles after one step; total momentum conserved over the step.  (K and V
+    at this size are not compared with the oracle: its O(N^2) V takes minutes here; config 2 at full size covers them.)"""
     w = inputs.TABLE23_WORKLOADS["ring_512k"]
     th, p = w.state()
     ctx = lrmd.Context(RING, w.N, w.eps)
