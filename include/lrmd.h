@@ -90,8 +90,11 @@ enum {
                                     shapes, 3 = cluster-resident kernel (N <= 20,480: state in registers of one
                                     thread-block cluster, all n steps of a call in one launch), 4 = grid-resident kernel
                                     (N <= 1,070,336: state in the shared memory of one CTA per SM, all n steps of a call
-                                    in one cooperative launch, a grid barrier per substage; falls back to 0 if the device
-                                    refuses the cooperative launch); -1 = choose from N (3 up to 20,480, 4 up to 1,070,336,
+                                    in one cooperative launch, a grid barrier per substage; if the device refuses the cooperative
+                                    launch — cudaErrorCooperativeLaunchTooLarge, NotSupported, InvalidValue or
+                                    InvalidConfiguration, e.g. under MPS with fewer SMs — the context switches to the substage
+                                    kernels for good and lrmd_get_option shows the variant then in use; any other CUDA error
+                                    is returned as LRMD_ECUDA); -1 = choose from N (3 up to 20,480, 4 up to 1,070,336,
                                     1 beyond; shards: 0 below 1e6, else 1)                                                  */
     LRMD_OPT_PAIR_VARIANT = 6,   /* pair models: launch shape of the pair kernels (-1 = choose).  Ordered kernels:
                                     0 = 128 threads x 4 rows, 1 = 128 x 8, 2 = 256 x 4.  Symmetric and band kernels:
@@ -101,21 +104,24 @@ enum {
                                     both particles (the paper declines this): 1 = warp-level
                                     kernel (one j-side scratch row per 32R-particle tile; fp64 and, GRAV2D, fp32 pairs),
                                     2 = band kernel (fp64, and GRAV2D fp32 pairs; both sides' sums kept on chip over blocks of 8 x 32R
-                                    particles, one launch for any N, about 25 N doubles of scratch per component);
+                                    particles, one launch for any N; scratch about 40 N doubles per component with the default band height —
+                                    673 MB at config 5, N = 2^20 — see lrmd_workspace_bytes);
                                     0 = every ordered pair (the paper's scheme); -1 = choose (1 for 2048 <= N < 49,152,
                                     2 beyond, 0 if the context is a shard).  get: the kernel in use.  With 1
                                     LRMD_OPT_PAIR_CTAS counts warps (workers) per launch, with 2 CTAs.                */
     LRMD_OPT_PAIR_SYM_TILES = 9, /* symmetric kernel: i-tiles per launch (0 = as many as keep the j-side scratch rows,
                                     N doubles per tile and component, within 1 GiB); get: the value in use            */
+    LRMD_OPT_PAIR_FUSE_UPDATE = 10, /* symmetric kernel, one launch per force evaluation: 0 = separate update kernel,
+                                    1 / -1 = the kick / drift that follows a force evaluation runs inside its fold
+                                    kernel (same arithmetic, bit-identical results); get: whether it is in use       */
     LRMD_OPT_PAIR_SYM_EXCHANGE = 11, /* symmetric fp64 kernel: how the j-packet (position + collected force) meets the lanes:
                                     0 = it travels around the warp by shuffles, 1-3 = it lives in a per-warp shared-memory
                                     buffer (register budget for 2, 3, 4 resident CTAs per SM); -1 = choose.  Results differ
                                     between 0 and 1-3 in the rounding of the j-side sums only.                        */
-    LRMD_OPT_PAIR_BAND_HEIGHT = 12, /* band kernel: I-blocks per band (0 = choose: the height that minimises the scratch
-                                    rows); get: the value in use                                                      */
-    LRMD_OPT_PAIR_FUSE_UPDATE = 10 /* symmetric kernel, one launch per force evaluation: 0 = separate update kernel,
-                                    1 / -1 = the kick / drift that follows a force evaluation runs inside its fold
-                                    kernel (same arithmetic, bit-identical results); get: whether it is in use       */
+    LRMD_OPT_PAIR_BAND_HEIGHT = 12  /* band kernel: I-blocks per band.  0 = choose: the tallest band whose i-side scratch rows,
+                                    which all CTAs cycle through, stay within 80 MB of the L2 (16 at config 5); only when
+                                    that choice would need more than 1 GiB of rows, the height that minimises the scratch
+                                    (N = 3e6: 24).  get: the value in use                                               */
 };
 
 /* Create a context for `model` (LRMD_HMF | LRMD_RING | LRMD_GRAV2D) with N >= 1 particles.
@@ -130,7 +136,11 @@ int lrmd_destroy(lrmd_ctx* ctx);
 /* Scratch needed for the current options: partial sums, the packed j-stream (cos,sin) or (x,y)
  * of PAPER.md:100, partial forces, device scalars.  Query, allocate `*bytes` on the device
  * (256-byte aligned), then bind it.  Changing an option that alters the size returns the
- * context to "workspace not set".  The contents are private to the library. */
+ * context to "workspace not set".  A context that uses a symmetric or band pair kernel keeps work tables
+ * in the workspace which every resolving call rebuilds: there ANY lrmd_set_option (except KERNEL_TIMING,
+ * PAIR_FUSE_UPDATE and PAIR_SYM_EXCHANGE) and any lrmd_set_shard returns the context to "workspace not
+ * set", even if the size did not change — call lrmd_set_workspace again (the next call otherwise returns
+ * LRMD_ESTATE).  The contents are private to the library. */
 int lrmd_workspace_bytes(const lrmd_ctx* ctx, size_t* bytes);
 /* lrmd_set_workspace copies the small work tables of the symmetric / band pair kernels (a few KB to a few MB, built on
  * the host when the options were resolved) into the workspace with cudaMemcpyAsync on cuda_stream and SYNCHRONISES
@@ -178,11 +188,12 @@ int lrmd_step_observe(lrmd_ctx* ctx, int64_t n, double dt, int64_t every, double
  * particles only.  The exchange steps are the caller's collectives (NCCL through torch.distributed in the Python
  * binding), called by the library on the stream between its kernels:
  *   HMF          after every reduction: allreduce(device pointer to this rank's (sum cos, sum sin), 2, stream, user)
- *                must sum the 2 doubles over all ranks in place ("each GPU computes its contribution to the
- *                magnetisation, which are then summed");
+ *                must sum the 2 doubles over all ranks in place (each GPU "computes the magnetization
+ *                components for its corresponding number of particles, and their sum give the total");
  *   RING/GRAV2D  after every drift: allgather(device pointer to the packed j-stream of ALL N_total particles,
  *                elem_bytes, i0, N, N_total, stream, user) — this rank's N elements are already in place at element
- *                offset i0; the callback must fill in the other ranks' ("each GPU holds all positions").
+ *                offset i0; the callback must fill in the other ranks' (each GPU stores half of the momenta
+ *                and forces "but all the particle position coordinates").
  * A callback returns 0 on success.  lrmd_energy on a shard returns this rank's part of K, of V (pair models: rows
  * owned x all j, halved) and of the momentum sums — add them over ranks; HMF's V, Mx, My are already global.
  * N_total = N (a single shard) restores the unsharded path.  Changes the workspace size. */

@@ -96,6 +96,9 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
             const int ncol = (int)((N - col0 < (long long)n * 32) ? (N - col0) : (long long)n * 32);   // columns that exist
             __syncthreads();    // the previous segment's shared-memory reads are done
             if (threadIdx.x == 0) {
+                // the previous segment's generic-proxy reads and zero-fill writes of Jpos, ordered before this thread by
+                // the barrier, must also be ordered before the bulk copy's async-proxy writes to the same addresses
+                fence_proxy_async_smem();
                 mbar_expect_tx(bar, (uint32_t)ncol * (uint32_t)sizeof(double2));
                 bulk_g2s(Jpos, js + col0, (uint32_t)ncol * (uint32_t)sizeof(double2), bar);
             }
@@ -304,6 +307,7 @@ grav_force_band_f32_kernel(const float2* __restrict__ js32, BandPart B, float ep
             const int ncopy = (ncol + 1) & ~1;        // bulk copies move multiples of 16 bytes (the stream is padded by 2)
             __syncthreads();
             if (threadIdx.x == 0) {
+                fence_proxy_async_smem();      // as in the fp64 kernel: generic accesses to Jpos before the async-proxy writes
                 mbar_expect_tx(bar, (uint32_t)ncopy * (uint32_t)sizeof(float2));
                 bulk_g2s(Jpos, js32 + col0, (uint32_t)ncopy * (uint32_t)sizeof(float2), bar);
             }

@@ -709,6 +709,13 @@ int hmf_step_cluster(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     return LRMD_OK;
 }
 
+// Errors that mean "this device will not run the grid-resident kernel" (too few SMs for one CTA each, no cooperative
+// launch, shared memory not granted); anything else is a real failure and is reported as LRMD_ECUDA.
+inline bool grid_refused(cudaError_t e) {
+    return e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported || e == cudaErrorInvalidValue ||
+           e == cudaErrorInvalidConfiguration;
+}
+
 // All n steps in one cooperative launch of one CTA per SM (hmf_grid_kernel).  Returns LRMD_EUNSUPPORTED if the device
 // refuses the cooperative launch (the caller then falls back to the substage kernels).
 int hmf_step_grid(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
@@ -721,7 +728,7 @@ int hmf_step_grid(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     if (!ready) {
         const cudaError_t ea = cudaFuncSetAttribute((const void*)hmf_grid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                     (int)((size_t)kHmfGridMaxLocal * kHmfGridBytesPerParticle));
-        if (ea != cudaSuccess) { c->cuda_err = (int)ea; (void)cudaGetLastError(); return LRMD_EUNSUPPORTED; }
+        if (ea != cudaSuccess) { c->cuda_err = (int)ea; (void)cudaGetLastError(); return grid_refused(ea) ? LRMD_EUNSUPPORTED : LRMD_ECUDA; }
         c->smem_ready.push_back((const void*)hmf_grid_kernel);
     }
     cudaLaunchConfig_t cfg;
@@ -748,7 +755,7 @@ int hmf_step_grid(lrmd_ctx* c, int64_t n, double dt, cudaStream_t stream) {
     const int nxt = (c->cur + 1) % 3;
     const cudaError_t e = cudaLaunchKernelEx(&cfg, hmf_grid_kernel, c->a0, c->a1, (long long)c->N, nlocal, (long long)n,
                                              k.B0 * dt, k.B1 * dt, k.D0 * dt, k.D1 * dt, hmf_buf(c, nxt), hmf_buf(c, c->cur));
-    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return LRMD_EUNSUPPORTED; }
+    if (e != cudaSuccess) { c->cuda_err = (int)e; (void)cudaGetLastError(); return grid_refused(e) ? LRMD_EUNSUPPORTED : LRMD_ECUDA; }
     if (t) { cudaEventRecord(c->ev[c->ev_used + 1], stream); c->ev_used += 2; }
     ++c->launches;
     c->force_valid = true;   // the kernel leaves the per-CTA sums at the final angles in the current partial buffer

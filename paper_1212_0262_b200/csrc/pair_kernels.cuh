@@ -274,9 +274,9 @@ pair_force_kernel(const double2* __restrict__ js, PairPart P, double eps, double
 }
 
 // ---- 2D force, fp32 pair arithmetic ----------------------------------
-// The paper's mixed-precision variant: "the positions are copied to single precision variables in
-// shared memory, the force is computed in single precision and then summed to a double precision
-// variable".  Here: a second packed stream float2 xy32[] (positions rounded to fp32 by the update
+// The paper's mixed-precision variant (paraphrased): all data stay in double precision in global
+// memory, each position component is stored in single precision in shared memory, the force between two particles
+// "is then computed in single precision but added in a double precision variable".  Here: a second packed stream float2 xy32[] (positions rounded to fp32 by the update
 // kernel), pair terms in fp32 (4 FADD/FFMA for dx, dy, r^2 + eps; MUFU.RCP; 2 FFMA), summed in fp32
 // over at most kF32Chunk consecutive j and then added to the fp64 accumulators (reading G16: a
 // pure fp32 accumulator over 1e6 terms would miss the 1e-5 tolerance).  Bound by the special-

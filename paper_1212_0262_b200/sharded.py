@@ -65,6 +65,7 @@ class ShardedContext(lrmd.Context):
 
     def __init__(self, model: int, n_total: int, eps: float, coll, device="cuda:0", options: dict | None = None):
         self.coll = coll
+        self.last_collective_error = None             # the exception behind the last LRMD_ECOLL, if any
         self.n_total = int(n_total)
         self.bounds = shard_bounds(self.n_total, coll.world)
         self.i0, n_local = self.bounds[coll.rank]
@@ -76,6 +77,14 @@ class ShardedContext(lrmd.Context):
         rc = lrmd.load().lrmd_set_shard(self._h, self.n_total, self.i0, self._ar, self._ag, None)
         self._chk(rc, "lrmd_set_shard")
         self._bind_workspace()
+
+    def _chk(self, rc, what):
+        """As Context._chk; an LRMD_ECOLL carries the exception the collective callback raised (it cannot cross the C
+        boundary, so the callback stores it and returns 1)."""
+        if rc == lrmd.ECOLL and self.last_collective_error is not None:
+            exc, self.last_collective_error = self.last_collective_error, None
+            raise lrmd.LrmdError(rc, "%s (collective callback raised %s: %s)" % (what, type(exc).__name__, exc)) from exc
+        super()._chk(rc, what)
 
     # -- views of the workspace the library hands back as raw device pointers
     def _view(self, ptr: int, nbytes: int):
@@ -101,7 +110,8 @@ class ShardedContext(lrmd.Context):
             with self._on_stream(stream):
                 self.coll.all_reduce_sum_(self._view(ptr, 8 * count).view(self._torch.float64))
             return 0
-        except Exception:          # never let an exception cross the C boundary
+        except Exception as exc:   # never let an exception cross the C boundary; kept for the LRMD_ECOLL report
+            self.last_collective_error = exc
             return 1
 
     def _allgather(self, ptr, elem_bytes, i0, n_local, n_total, stream, user):
@@ -110,7 +120,8 @@ class ShardedContext(lrmd.Context):
             with self._on_stream(stream):
                 self.coll.all_gather_inplace_(whole, [(b * elem_bytes, (b + n) * elem_bytes) for b, n in self.bounds])
             return 0
-        except Exception:
+        except Exception as exc:
+            self.last_collective_error = exc
             return 1
 
     def set_state_global(self, *arrays):

@@ -144,3 +144,30 @@ def test_single_shard_is_the_unsharded_path(lrmd):
     assert lrmd.load().lrmd_set_shard(h, 5, 0, None, None, None) == lrmd.EINVAL      # N_total < N
     lrmd.lrmd_destroy(h)
     a.close(); b.close()
+
+
+class _FailingColl:
+    """One rank that claims to be rank 0 of 2; its collectives raise."""
+    rank, world = 0, 2
+
+    def all_reduce_sum_(self, t):
+        raise RuntimeError("link down (all_reduce)")
+
+    def all_gather_inplace_(self, whole, byte_bounds):
+        raise RuntimeError("link down (all_gather)")
+
+
+@pytest.mark.parametrize("model,what", [(HMF, "all_reduce"), (GRAV2D, "all_gather")])
+def test_a_failing_collective_surfaces_with_its_message(model, what):
+    """A collective callback that raises cannot let the exception cross the C boundary: the library returns LRMD_ECOLL
+    and the binding re-raises with the original exception attached, instead of a bare error code."""
+    from paper_1212_0262_b200 import lrmd, sharded
+    N = 4096
+    ctx = sharded.ShardedContext(model, N, 0.0 if model == HMF else 1e-3, _FailingColl())
+    rng = np.random.default_rng(3)
+    ctx.set_state(*[rng.uniform(-1, 1, ctx.N) for _ in range(ctx.narrays)])
+    with pytest.raises(lrmd.LrmdError) as ei:
+        ctx.step(1, 0.01)
+    assert ei.value.code == lrmd.ECOLL and "link down (%s)" % what in str(ei.value)
+    assert isinstance(ei.value.__cause__, RuntimeError)
+    ctx.close()
