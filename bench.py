@@ -60,16 +60,16 @@ SYM_PAIR_FP64_INSTR = {1: 6.0, 2: 5.5}
 HMF_BYTES_PER_PARTICLE_SUBSTAGE = 32.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel come from the committed
-# `ncu --set full` captures: profiles/r02_traffic.csv names, per bench entry, the kernel, the two byte counts and
-# the capture they were read from (profiles/r02_ncu_full.md gives the commands).
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+# `ncu --set full` captures: profiles/r03_traffic.csv names, per bench entry, the kernel, the two byte counts and
+# the capture they were read from (profiles/r03_ncu.md and profiles/r02_ncu_full.md give the commands).
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic.csv")
 
 
 def ncu_traffic(entry, kernel):
-    """(bytes per launch, source) of `kernel` in bench entry `entry` from profiles/r02_traffic.csv, or (None, why)."""
+    """(bytes per launch, source) of `kernel` in bench entry `entry` from profiles/r03_traffic.csv, or (None, why)."""
     import csv
     if not os.path.exists(TRAFFIC_CSV):
-        return None, "profiles/r02_traffic.csv missing"
+        return None, "profiles/r03_traffic.csv missing"
     with open(TRAFFIC_CSV) as fh:
         for row in csv.DictReader(fh):
             if row["entry"] == entry:
