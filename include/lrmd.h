@@ -116,8 +116,12 @@ enum {
                                     kernel (same arithmetic, bit-identical results); get: whether it is in use       */
     LRMD_OPT_PAIR_SYM_EXCHANGE = 11, /* symmetric fp64 kernel: how the j-packet (position + collected force) meets the lanes:
                                     0 = it travels around the warp by shuffles, 1-3 = it lives in a per-warp shared-memory
-                                    buffer (register budget for 2, 3, 4 resident CTAs per SM); -1 = choose.  Results differ
-                                    between 0 and 1-3 in the rounding of the j-side sums only.                        */
+                                    buffer (register budget for 2, 3, 4 resident CTAs per SM); -1 = choose (3).  fp32 band
+                                    kernel (GRAV2D, pair precision 1): 0 = the j-side sum of a slot is an fp32 packet that
+                                    travels with the slot by shuffles and joins the fp64 sum once per 32-step visit (fp32
+                                    over 32 R terms), 1-3 = it joins the slot's fp64 sum in shared memory every step (fp32
+                                    over R terms); -1 = choose (0).  Results differ between 0 and 1-3 in the rounding of
+                                    the j-side sums only.                                                             */
     LRMD_OPT_PAIR_BAND_HEIGHT = 12  /* band kernel: I-blocks per band.  0 = choose: the tallest band whose i-side scratch rows,
                                     which all CTAs cycle through, stay within 80 MB of the L2 (16 at config 5); only when
                                     that choice would need more than 1 GiB of rows, the height that minimises the scratch

@@ -226,24 +226,30 @@ pair_force_band_kernel(const double2* __restrict__ js, BandPart B, double eps, d
 // packet in shared memory: per step the lane adds the fp32 sum of its R terms to the slot's fp64 sum (reading G16: fp32
 // sums never run over more than R terms on the j side, 32 on the i side).  64 registers of state per thread instead of
 // the warp-level kernel's 191: 16 resident warps per SM instead of 8.
-template <int R, bool MASK, bool DIAG>
+template <int R, bool MASK, bool DIAG, bool JSHFL = false>
 __device__ __forceinline__ void sym_chunk_f32_smem(const float (&a)[R], const float (&b)[R], const bool (&vi)[R],
                                                    double (&f0)[R], double (&f1)[R], const float2* __restrict__ spos,
                                                    double2* __restrict__ sg, int nvalid, float eps) {
+    // JSHFL (LRMD_OPT_PAIR_SYM_EXCHANGE = 0): the j-side sum of the slot a lane faces is an fp32 packet that travels with
+    // the slot from lane to lane (at step s lane l faces slot l + s, which lane l + 1 faced the step before) and is added
+    // to the slot's fp64 sum ONCE per visit: 2 SHFL per step instead of LDS.128 + 2 F2F + 2 DADD + STS.128 + a warp
+    // barrier — the two conversions share the 16-lane XU pipe with the R MUFU.RCP of the step.  The fp32 packet then runs
+    // over 32 R terms (256 for R = 8) instead of R; the sums across visits stay fp64 (reading G16).
     const int lane = threadIdx.x & 31;
     float sx[R], sy[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) sx[r] = sy[r] = 0.f;
     float2 qn = spos[lane];
+    float h0 = 0.f, h1 = 0.f;
 #pragma unroll 4
     for (int s = 0; s < 32; ++s) {
         const int idx = (lane + s) & 31;
         const float2 q = qn;
         qn = spos[(idx + 1) & 31];
         double2 g = make_double2(0.0, 0.0);
-        if (!DIAG) g = sg[idx];
+        if (!DIAG && !JSHFL) g = sg[idx];
         const bool vq = MASK ? (idx < nvalid) : true;
-        float h0 = 0.f, h1 = 0.f;
+        if (!JSHFL) { h0 = 0.f; h1 = 0.f; }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float dx = a[r] - q.x, dy = b[r] - q.y;
@@ -258,9 +264,22 @@ __device__ __forceinline__ void sym_chunk_f32_smem(const float (&a)[R], const fl
             }
         }
         if (!DIAG) {
-            sg[idx] = make_double2(g.x + (double)h0, g.y + (double)h1);
-            __syncwarp();
+            if (JSHFL) {
+                if (s < 31) {       // hand the packet to the lane that faces this slot next
+                    h0 = __shfl_sync(0xffffffffu, h0, (lane + 1) & 31);
+                    h1 = __shfl_sync(0xffffffffu, h1, (lane + 1) & 31);
+                }
+            } else {
+                sg[idx] = make_double2(g.x + (double)h0, g.y + (double)h1);
+                __syncwarp();
+            }
         }
+    }
+    if (!DIAG && JSHFL) {
+        const int idx = (lane + 31) & 31;       // the slot faced at the last step: its packet is complete
+        const double2 g = sg[idx];
+        sg[idx] = make_double2(g.x + (double)h0, g.y + (double)h1);
+        __syncwarp();
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {
@@ -274,7 +293,7 @@ constexpr size_t band_f32_smem_bytes(int R) { return (size_t)kBandWarps * 32 * R
 // (R = 16, launch shape 2: 255 registers, one CTA per SM; 3.5 % faster than R = 8 at N = 102,400, not the default.
 //  Packed fp32x2 arithmetic (FADD2 / FFMA2) was tried for the walk and measured 5 % slower: the packed instructions
 //  issue at half rate and the pair packing costs register moves.)
-template <int R>
+template <int R, bool JSHFL = false>
 __global__ void __launch_bounds__(kBandThreads, (R <= 8 ? 2 : 1))
 grav_force_band_f32_kernel(const float2* __restrict__ js32, BandPart B, float eps, double pre, double* __restrict__ ibuf0,
                            double* __restrict__ ibuf1, double* __restrict__ jbuf0, double* __restrict__ jbuf1) {
@@ -349,11 +368,11 @@ grav_force_band_f32_kernel(const float2* __restrict__ js32, BandPart B, float ep
                         const float2* sp = Jpos + x * 32;
                         double2* sg = Jg + x * 32;
                         if (diag) {
-                            if (masked) sym_chunk_f32_smem<R, true, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
-                            else sym_chunk_f32_smem<R, false, true>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            if (masked) sym_chunk_f32_smem<R, true, true, JSHFL>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            else sym_chunk_f32_smem<R, false, true, JSHFL>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
                         } else {
-                            if (masked) sym_chunk_f32_smem<R, true, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
-                            else sym_chunk_f32_smem<R, false, false>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            if (masked) sym_chunk_f32_smem<R, true, false, JSHFL>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
+                            else sym_chunk_f32_smem<R, false, false, JSHFL>(a, bb, vi, f0, f1, sp, sg, nvalid, eps);
                         }
                     }
                     if (!diag && (k + 1) % m == 0 && k + 1 < nv) __syncthreads();

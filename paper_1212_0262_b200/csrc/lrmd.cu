@@ -885,9 +885,14 @@ void pair_force_band(Launcher& L, int upd = 0, double kickA = 0.0, double kickB 
     const dim3 g((unsigned)c->bpart.P), b(kBandThreads);
     if (c->opt_precision == 1) {
         L.smem = band_f32_smem_bytes(c->band_R);
-        if (c->band_R == 16) L.go_timed(grav_force_band_f32_kernel<16>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
-        else if (c->band_R == 8) L.go_timed(grav_force_band_f32_kernel<8>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
-        else L.go_timed(grav_force_band_f32_kernel<4>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1);
+#define LRMD_BAND32_GO(RR, X) L.go_timed(grav_force_band_f32_kernel<RR, X>, g, b, (const float2*)js32_ptr(c), c->bpart, (float)c->eps, pre, i0, i1, j0, j1)
+        // LRMD_OPT_PAIR_SYM_EXCHANGE 0 / -1 (default): the j-side fp32 packet travels by shuffles, one fp64 add per chunk
+        // visit (11 % faster at N = 2^20 than 1-3, the per-step shared-memory exchange; worst error 4e-8 A_i either way)
+        const bool jshfl = c->opt_sym_xch <= 0;
+        if (c->band_R == 16) { if (jshfl) LRMD_BAND32_GO(16, true); else LRMD_BAND32_GO(16, false); }
+        else if (c->band_R == 8) { if (jshfl) LRMD_BAND32_GO(8, true); else LRMD_BAND32_GO(8, false); }
+        else { if (jshfl) LRMD_BAND32_GO(4, true); else LRMD_BAND32_GO(4, false); }
+#undef LRMD_BAND32_GO
         withv = false;
     } else {
     L.smem = band_smem_bytes(c->band_R);
@@ -1468,7 +1473,10 @@ int lrmd_get_option(const lrmd_ctx* c, int key, int64_t* value) {
         case LRMD_OPT_GRAPH: *value = c->use_graph ? 1 : 0; break;
         case LRMD_OPT_HMF_GRID: *value = c->hmf_grid; break;
         case LRMD_OPT_KERNEL_TIMING: *value = c->timing ? 1 : 0; break;
-        case LRMD_OPT_PAIR_SYM_EXCHANGE: *value = c->sym ? c->sym_xch : 0; break;
+        case LRMD_OPT_PAIR_SYM_EXCHANGE:
+            if (c->band && c->opt_precision == 1) *value = c->opt_sym_xch <= 0 ? 0 : c->sym_xch;     // fp32 band kernel
+            else *value = c->sym ? c->sym_xch : 0;
+            break;
         default: return LRMD_EINVAL;
     }
     return LRMD_OK;

@@ -177,9 +177,10 @@ def test_band_f32_pair_variant_forces(lrmd, ref, torch, N, variant):
     even number of elements), any number of workers and band heights; bitwise reproducible."""
     st = _state(GRAV2D, N, 950 + N % 13)
     f0, f1, A0, A1 = ref.forces_abs(GRAV2D, 1e-3, st[0], st[1], form=0)
-    for workers, height in ((0, 0), (3, 1), (37, 2)):
+    # exchange -1 / 0: the j-side fp32 packet travels by shuffles (default); 1: it joins the fp64 slot sum every step
+    for workers, height, xch in ((0, 0, -1), (3, 1, 0), (37, 2, -1), (0, 0, 1), (37, 2, 1)):
         opts = {lrmd.OPT_PAIR_PRECISION: 1, lrmd.OPT_PAIR_SYMMETRIC: 2, lrmd.OPT_PAIR_VARIANT: variant,
-                lrmd.OPT_PAIR_CTAS: workers, lrmd.OPT_PAIR_BAND_HEIGHT: height}
+                lrmd.OPT_PAIR_CTAS: workers, lrmd.OPT_PAIR_BAND_HEIGHT: height, lrmd.OPT_PAIR_SYM_EXCHANGE: xch}
         got = _forces(lrmd, GRAV2D, N, 1e-3, st, opts)
         again = _forces(lrmd, GRAV2D, N, 1e-3, st, opts)
         for g, h, w, a in ((got[0], again[0], f0, A0), (got[1], again[1], f1, A1)):
